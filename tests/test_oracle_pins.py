@@ -1,0 +1,520 @@
+"""Pins for oracle/ (CPU only).  Each test fixes a part of the oracle to something OTHER than the
+oracle itself: published known-answer vectors, closed forms, invariants, special cases that reduce
+to a textbook routine, or brute force in independent exact / high-precision arithmetic.
+Pin numbers P1..P12 and steps S0..S14 refer to SURVEY.md section 8(c); P:Lnnn = PAPER.md line nnn.
+"""
+import decimal
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle as O
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+GOLD = os.path.join(HERE, "golden")
+SR = 44100
+
+
+# ----------------------------------------------------------------------------- helpers
+def read_kv(path):
+    out = {}
+    for line in open(path):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        k, v = line.split("=", 1)
+        out[k.strip()] = v.strip()
+    return out
+
+
+def fixed_nebula(h):
+    """A nebula with lo = hi = h[p]: map() then returns h[p] exactly for any u (S3)."""
+    neb = np.zeros(O.NPARAM, dtype=O.NEBULA_DTYPE)
+    neb["lo"] = h
+    neb["hi"] = h
+    neb["curve"] = 1.0
+    neb["symmetric"] = 0
+    return neb
+
+
+def neutral_h(D=100.0):
+    """Human-unit parameter vector (layout S2) in which everything is switched off/flat:
+    all six ADSRs are a constant 1 while t < D (A = Dc = Rl = 0, S = 1, alpha = 1)."""
+    h = np.zeros(O.NPARAM)
+    h[0], h[1] = 69.0, D
+    for e in range(6):
+        h[2 + 5 * e: 7 + 5 * e] = [0.0, 0.0, 1.0, 0.0, 1.0]
+    for l in range(2):
+        h[32 + 8 * l: 40 + 8 * l] = [0.0, 0.0, 0.0, 1.0, 0.0, 0.0, 0.0, 0.0]
+    return h
+
+
+def render_h(h, N, sr=SR, noise_key=(1, 2), want_phase=False):
+    u = np.full(O.NPARAM, 0.5, dtype=np.float32)
+    return O.render_voice(u, np.array(noise_key, dtype=np.uint32), sr, N, fixed_nebula(h), want_phase=want_phase)
+
+
+def py_philox(ctr, key):
+    """Independent re-statement of S0 in Python integers (itself checked against the KATs below)."""
+    c = list(ctr); k = list(key)
+    for r in range(10):
+        if r:
+            k[0] = (k[0] + 0x9E3779B9) & 0xFFFFFFFF
+            k[1] = (k[1] + 0xBB67AE85) & 0xFFFFFFFF
+        p0 = 0xD2511F53 * c[0]; p1 = 0xCD9E8D57 * c[2]
+        c = [(p1 >> 32) ^ c[1] ^ k[0], p1 & 0xFFFFFFFF, (p0 >> 32) ^ c[3] ^ k[1], p0 & 0xFFFFFFFF]
+    return c
+
+
+def kat_vectors():
+    rows = []
+    for line in open(os.path.join(GOLD, "philox_kat.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        w = [int(x, 16) for x in line.split()]
+        rows.append((w[0:4], w[4:6], w[6:10]))
+    return rows
+
+
+# ----------------------------------------------------------------------------- P1 Philox
+def test_p1_philox_known_answer_vectors():
+    rows = kat_vectors()
+    assert len(rows) == 3
+    for ctr, key, want in rows:
+        assert list(O.philox4x32_10(ctr, key)) == want
+        assert py_philox(ctr, key) == want
+
+
+def test_p1_philox_vs_independent_python_random_inputs():
+    rng = np.random.default_rng(1)
+    for _ in range(200):
+        ctr = [int(x) for x in rng.integers(0, 2**32, 4)]
+        key = [int(x) for x in rng.integers(0, 2**32, 2)]
+        assert list(O.philox4x32_10(ctr, key)) == py_philox(ctr, key)
+
+
+# ----------------------------------------------------------------------------- P2 sampler layout
+def test_p2_sampler_block0_follows_from_kat():
+    # seed 0, g 0, block 0 is ctr = 0, key = 0: the first KAT line.  u = (word >> 8) * 2^-24 (S1, D5)
+    u, nk = O.sample_params(0, 0, 1)
+    want = [(w >> 8) / 2.0**24 for w in kat_vectors()[0][2]]
+    assert [float(x) for x in u[0, :4]] == want
+
+
+def test_p2_sampler_survey_probe_values():
+    g = read_kv(os.path.join(GOLD, "survey_probe.txt"))
+    u, nk = O.sample_params(0, 0, 1)
+    for i in range(4):
+        assert float(u[0, i]) == float(g[f"u{i}"])
+    b19 = [int(x, 16) for x in g["block19"].split()]
+    assert [int(round(float(x) * 2**24)) for x in u[0, 76:78]] == [w >> 8 for w in b19[:2]]
+    assert [int(x) for x in nk[0]] == [int(x, 16) for x in g["noise_key"].split()]
+    nb = [int(x, 16) for x in g["noise_block0"].split()]
+    assert [O.noise_word(nk[0], n) for n in range(4)] == nb
+    z = [float(x) for x in g["noise_z0"].split()]
+    assert np.allclose([O.noise_value(w) for w in nb], z, atol=5e-9)
+    u7, _ = O.sample_params(7, 3, 128)  # g = 3*128 + 5 = 389
+    s7 = [int(x, 16) for x in g["seed7_g389_block0"].split()]
+    assert [int(round(float(x) * 2**24)) for x in u7[5, :4]] == [w >> 8 for w in s7]
+
+
+def test_p2_sampler_counter_and_key_layout_64bit():
+    # ctr = (block, g lo32, g hi32, stream), key = (seed lo32, seed hi32): exercised with hi parts set
+    seed = (0xDEADBEEF << 32) | 0x12345678
+    g = (0x3 << 32) | 0x9ABCDEF0
+    u, nk = O.sample_params(seed, g, 1)  # batch_index*B + b with B = 1
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    for p in range(O.NPARAM):
+        w = py_philox([p >> 2, g & 0xFFFFFFFF, g >> 32, 0], key)[p & 3]
+        assert float(u[0, p]) == (w >> 8) / 2.0**24
+    assert [int(x) for x in nk[0]] == py_philox([0, g & 0xFFFFFFFF, g >> 32, 2], key)[:2]
+
+
+def test_p2_u_on_24bit_grid_and_uniform():
+    u, _ = O.sample_params(0, 0, 512)
+    x = u.astype(np.float64) * 2**24
+    assert np.all(x == np.round(x)) and x.min() >= 0 and x.max() < 2**24
+    # P:L143 "sampled uniformly": mean 1/2, var 1/12 over 512*78 draws (4-sigma bands)
+    n = u.size
+    assert abs(u.mean() - 0.5) < 4 * math.sqrt(1 / 12 / n)
+    assert abs(u.var() - 1 / 12) < 4 * math.sqrt(1 / 180 / n)
+
+
+def test_p3_sampler_b_invariance():
+    a, ka = O.sample_params(5, 0, 256)
+    b, kb = O.sample_params(5, 1, 128)
+    assert np.array_equal(a[128:], b) and np.array_equal(ka[128:], kb)
+
+
+# ----------------------------------------------------------------------------- P4 map
+def test_p4_map_closed_forms():
+    assert O.map_param(0.0, -3, 9, 0.37, 0) == -3 and O.map_param(1.0, -3, 9, 0.37, 0) == 9
+    assert O.map_param(0.25, -3, 9, 1.0, 0) == 0.0                       # affine
+    assert O.map_param(0.5, 0, 2, 0.5, 0) == 0.5                         # 2 * 0.5^2
+    assert O.map_param(0.5, -24, 24, 0.2, 1) == 0.0                      # symmetric centre, exact
+    assert O.map_param(0.0, -96, 96, 0.2, 1) == -96 and O.map_param(1.0, -96, 96, 0.2, 1) == 96
+    assert O.map_param(0.75, -10, 10, 0.5, 1) == pytest.approx(10 * 0.25, abs=1e-15)  # (2u-1)^2 = .25
+    assert O.map_param(0.25, -10, 10, 0.5, 1) == pytest.approx(-10 * 0.25, abs=1e-15)
+    assert O.map_param(0.75, -10, 10, 1.0, 1) == 5.0
+    # clamp (8(b)): out-of-range and NaN behave as the nearest end / 0
+    assert O.map_param(-1, 0, 2, 0.5, 0) == 0 and O.map_param(7, 0, 2, 0.5, 0) == 2
+    assert O.map_param(float("nan"), 1, 2, 1, 0) == 1
+
+
+@pytest.mark.parametrize("c", [0.1, 0.25, 0.5, 1.0, 3.0, 10.0])
+def test_p4_map_monotone_and_inverse_round_trip(c):
+    us = np.linspace(0, 1, 201)
+    for sym in (0, 1):
+        # lo = 0 (centre 0 when symmetric) so that tiny u^(1/c) is not absorbed by the offset
+        lo, hi = (-4.0, 4.0) if sym else (0.0, 8.0)
+        hs = np.array([O.map_param(u, lo, hi, c, sym) for u in us])
+        assert np.all(np.diff(hs) >= 0)
+        for u, h in zip(us, hs):
+            if sym:
+                d = h / 4.0
+                back = (math.copysign(abs(d) ** c, d) + 1) / 2
+            else:
+                back = (h / 8.0) ** c
+            assert back == pytest.approx(u, abs=1e-9)
+
+
+def test_p4_c_below_one_favours_low_or_centre():
+    assert O.map_param(0.5, 0, 1, 0.25, 0) < 0.5 < O.map_param(0.5, 0, 1, 4.0, 0)
+    assert abs(O.map_param(0.75, -1, 1, 0.25, 1)) < 0.5 < abs(O.map_param(0.75, -1, 1, 4.0, 1))
+
+
+def test_s2_default_nebula_matches_baseline_ranges_and_count():
+    neb = O.default_nebula()
+    assert len(neb) == 78
+    rng = lambda i: (neb["lo"][i], neb["hi"][i])
+    assert rng(0) == (0, 127) and rng(1) == (0.01, 1.0)                       # BASELINE.json configs[0]
+    for e in range(6):
+        b = 2 + 5 * e
+        assert rng(b) == rng(b + 1) == rng(b + 3) == (0, 2) and rng(b + 2) == (0, 1) and rng(b + 4) == (0.1, 6)
+    for l in range(2):
+        b = 32 + 8 * l
+        assert rng(b) == (0, 20) and rng(b + 1) == (-10, 10) and rng(b + 2) == (-0.5, 0.5)
+        assert neb["symmetric"][b + 1] == 1
+    for v in range(2):
+        b = 68 + 3 * v
+        assert rng(b) == (-24, 24) and rng(b + 1) == (-96, 96) and rng(b + 2) == (-0.5, 0.5)
+        assert neb["symmetric"][b] == 1 and neb["symmetric"][b + 1] == 1
+    for i in list(range(35, 40)) + list(range(43, 68)) + [74, 75, 76, 77]:
+        assert rng(i) == (0, 1)
+    assert np.all((neb["curve"] >= 0.1) & (neb["curve"] <= 10))               # P:L270 range of curve
+
+
+# ----------------------------------------------------------------------------- P5 ADSR
+def test_p5_adsr_segment_values():
+    A, Dc, S, Rl, al, D = .3, .2, .6, .4, 2.5, 1.0
+    f = lambda t: O.adsr(t, A, Dc, S, Rl, al, D)
+    assert f(0) == 0 and f(A) == 1
+    assert f(A + Dc) == pytest.approx(S, abs=1e-15) and f(.8) == pytest.approx(S, abs=1e-15)
+    assert f(D) == pytest.approx(S, abs=1e-15)
+    assert f(A / 2) == pytest.approx(0.5 ** al, abs=1e-15) == pytest.approx(0.176776695296637, abs=1e-14)
+    assert f(D + Rl / 2) == pytest.approx(S * (1 - 0.5 ** al), abs=1e-15) == pytest.approx(0.493933982822018, abs=1e-14)
+    assert f(D + Rl + 1e-9) == 0 and f(3.0) == 0
+    assert abs(f(D + Rl)) <= 1e-15
+    assert f(A + Dc / 2) == pytest.approx(1 - (1 - S) * 0.5 ** al, abs=1e-15)
+
+
+def test_p5_adsr_degenerate_and_early_note_off():
+    assert O.adsr(0, 0, .2, .6, .4, 2.5, 1.0) == 1                          # A = 0: step already 1 at t = 0
+    assert O.adsr(0.0, 0, 0, .6, .4, 2.5, 1.0) == pytest.approx(.6)         # A = Dc = 0: sustain at once
+    assert O.adsr(1.0, .1, .1, .5, 0, 1.0, 1.0) == 0                        # Rl = 0: off at t = D
+    assert O.adsr(.2, .3, .2, .6, .4, 1.0, .1) == pytest.approx((.2 / .3) * (1 - .1 / .4), abs=1e-15)  # = 0.5
+    ts = np.linspace(0, 2, 401)
+    lin = np.array([O.adsr(t, .5, .5, .5, .5, 1.0, 1.0) for t in ts])        # alpha = 1: piecewise linear
+    want = np.where(ts <= .5, ts / .5, np.where(ts <= 1.0, 1 - .5 * (ts - .5) / .5, .5 * (1 - np.clip((ts - 1) / .5, 0, 1))))
+    assert np.allclose(lin, want, atol=1e-14)
+    rng = np.random.default_rng(0)
+    for _ in range(300):
+        A, Dc, Rl = rng.uniform(0, 2, 3); S = rng.uniform(); al = rng.uniform(.1, 6); D = rng.uniform(.01, 1)
+        v = [O.adsr(t, A, Dc, S, Rl, al, D) for t in rng.uniform(0, 4, 8)]
+        assert min(v) >= 0 and max(v) <= 1
+
+
+# ----------------------------------------------------------------------------- P6 LFO / controls
+def test_p6_lfo_shape_table():
+    want = {0.0: [0, 0, -1, 1, 1], 0.25: [1, 1, -.5, .5, 1], 0.5: [0, 0, 0, 0, -1], 0.75: [-1, -1, .5, -.5, -1]}
+    for p, w in want.items():
+        assert np.allclose(O.lfo_shapes(p), w, atol=3e-16)
+
+
+def test_p6_lfo_constant_rate_closed_form_and_one_hot():
+    N = 4 * SR
+    cr = SR / 100
+    for shape, fn in [(2, lambda p: 2 * p - 1), (3, lambda p: 1 - 2 * p), (4, lambda p: np.where(p < .5, 1.0, -1.0)),
+                      (0, lambda p: np.sin(2 * np.pi * p)), (1, lambda p: 4 * np.abs(((p + .75) % 1) - .5) - 1)]:
+        h = neutral_h()
+        h[32] = 3.7; h[33] = 0.0; h[34] = 0.125
+        h[35:40] = 0; h[35 + shape] = 0.8
+        h[48 + 4 * 0 + 2] = 1.0   # vco1 pitch row <- lfo1 only
+        E, L, M = O.controls(h, SR, N)
+        j = np.arange(O.num_ticks(N))
+        p = (0.125 + j * 3.7 / cr) % 1.0           # depth = 0  =>  q_j = q_0 + j f / cr  (exclusive sum)
+        ok = np.abs(p - 0.5) > 1e-9                 # keep clear of the square's jump
+        assert np.allclose(L[0][ok], fn(p)[ok], atol=1e-11)
+        assert np.allclose(M[0][ok], fn(p)[ok], atol=1e-11)   # one-hot mod-mixer row passes the source
+        assert np.all(M[1:] == 0)                    # rows with zero weights are exactly 0 (S7)
+
+
+def test_p6_lfo_rate_and_amp_modulation_by_dedicated_adsrs():
+    # each LFO has a rate-mod and an amp-mod ADSR.  Rate ADSR = linear attack over 1 s:
+    # f(t) = f0 + dep * t  =>  q_j = q0 + sum_{i<j} (f0 + dep*i/cr)/cr  (arithmetic series, exclusive)
+    h = neutral_h()
+    h[32], h[33], h[34] = 2.0, 5.0, 0.0
+    h[35:40] = [0, 0, 1, 0, 0]                      # saw = 2p - 1: reads the phase back directly
+    h[2 + 5 * 3: 7 + 5 * 3] = [1.0, 0, 1, 0, 1]     # lfo1_rate ADSR: A = 1 s, alpha = 1
+    h[2 + 5 * 2: 7 + 5 * 2] = [0.5, 0, 1, 0, 1]     # lfo1_amp ADSR: A = 0.5 s, alpha = 1
+    N = SR
+    cr = SR / 100
+    E, L, M = O.controls(h, SR, N)
+    j = np.arange(O.num_ticks(N))
+    assert np.allclose(E[3], np.minimum(j / cr, 1.0), atol=1e-15)
+    q = 2.0 * j / cr + 5.0 * (j * (j - 1) / 2) / cr**2
+    jj = j[j <= cr]
+    amp = np.minimum(jj / cr / 0.5, 1.0)
+    assert np.allclose(L[0][jj], amp * (2 * (q[jj] % 1.0) - 1), atol=1e-10)
+
+
+def test_s7_modmix_weighted_mean():
+    h = neutral_h()
+    h[2:7] = [0, 0, 0.25, 0, 1]      # adsr1 == 0.25
+    h[7:12] = [0, 0, 0.75, 0, 1]     # adsr2 == 0.75
+    h[48 + 4 * 3 + 0] = 1.0; h[48 + 4 * 3 + 1] = 3.0   # vco2 amp row
+    E, L, M = O.controls(h, SR, 1000)
+    assert np.allclose(M[3], (1 * .25 + 3 * .75) / 4, atol=1e-16)
+
+
+# ----------------------------------------------------------------------------- P7 upsample
+def test_p7_upsample():
+    C = np.array([1.0, 3.0, -2.0, 0.5])
+    assert [O.upsample(C, 100 * j) for j in range(3)] == [1.0, 3.0, -2.0]
+    assert O.upsample(C, 150) == pytest.approx(0.5) and O.upsample(C, 25) == 1.5
+    lin = 0.125 * np.arange(5) - 0.25
+    assert all(O.upsample(lin, n) == pytest.approx(0.125 * n / 100 - 0.25, abs=1e-16) for n in range(400))
+
+
+# ----------------------------------------------------------------------------- P8 VCO / phase scan
+def sine_only_h(midi=69.0, phase=0.0):
+    h = neutral_h()
+    h[0] = midi; h[70] = phase
+    h[48 + 4 * 1 + 0] = 1.0      # vco1 amp row <- adsr1 == 1
+    h[75] = 1.0                  # mixer: vco1 only
+    return h
+
+
+def test_p8_constant_frequency_sine_is_sin_2pi_f_t():
+    N = 4410
+    a = render_h(sine_only_h(), N)["audio"]
+    n = np.arange(N)
+    assert np.abs(a - np.sin(2 * np.pi * 440.0 * n / SR)).max() < 1e-12
+    a = render_h(sine_only_h(phase=0.25), N)["audio"]         # phases are in cycles (D12)
+    assert np.abs(a - np.cos(2 * np.pi * 440.0 * n / SR)).max() < 1e-12
+    a = render_h(sine_only_h(midi=81.0), N)["audio"]          # one octave up: A5 = 880 Hz (D13)
+    assert np.abs(a - np.sin(2 * np.pi * 880.0 * n / SR)).max() < 1e-12
+
+
+def test_p8_period_exactly_100_samples_at_441_hz():
+    midi = 69 + 12 * math.log2(441 / 440)
+    a = render_h(sine_only_h(midi=midi), 20000)["audio"]
+    assert np.abs(a[100:] - a[:-100]).max() < 1e-11
+    assert np.abs(a[::100]).max() < 1e-11                     # exclusive sum: sample 0 uses phi_0 = 0
+
+
+def test_p8_dyadic_increment_phase_is_exact():
+    # sr = 3520, MIDI 69 => inc = 440/3520 = 1/8 exactly: phi_n = frac(phi_0 + n/8) with no rounding at all
+    r = render_h(sine_only_h(phase=0.0625), 64, sr=3520, want_phase=True)
+    assert np.array_equal(r["phase1"], (0.0625 + np.arange(64) / 8.0) % 1.0)
+    h = sine_only_h(midi=69 + 24); h[68] = -12.0              # tune adds in semitones: net one octave up
+    r = render_h(h, 64, sr=3520, want_phase=True)
+    assert np.array_equal(r["phase1"], (np.arange(64) / 4.0) % 1.0)
+
+
+def _swept_h():
+    h = sine_only_h(midi=60.0, phase=-0.3)
+    h[2:7] = [0.02, 0.01, 0.4, 0.0, 1.7]   # adsr1 moves within the first ticks
+    h[69] = 31.0                           # vco1 mod depth (st)
+    h[48 + 4 * 0 + 0] = 1.0                # vco1 pitch row <- adsr1
+    return h
+
+
+def test_p8_brute_force_cumulative_sum_high_precision():
+    """phi_n = phi_0 + sum_{k<n} (440/sr) 2^((pitch_k - 69)/12), pitch from upsampled control, re-done in
+    50-digit decimal arithmetic from the oracle's own tick values (pins S8 + S9 against a dropped term,
+    inclusive/exclusive slip, wrong sign or a semitone/octave mix-up)."""
+    h = _swept_h()
+    sr, N = 8000, 260
+    E, L, M = O.controls(h, sr, N)
+    r = render_h(h, N, sr=sr, want_phase=True)
+    decimal.getcontext().prec = 50
+    Dm = decimal.Decimal
+    phi = Dm(h[70])
+    ln2 = Dm(2).ln()
+    for n in range(N):
+        assert abs(float(phi % 1) - r["phase1"][n]) < 1e-13 or abs(abs(float(phi % 1) - r["phase1"][n]) - 1) < 1e-13
+        j, m = divmod(n, 100)
+        ctl = Dm(M[0][j]) + (Dm(M[0][j + 1]) - Dm(M[0][j])) * Dm(m) / Dm(100)
+        pitch = Dm(h[0]) + Dm(h[68]) + Dm(h[69]) * ctl
+        phi += Dm(440) / Dm(sr) * ((pitch - 69) / 12 * ln2).exp()
+
+
+def test_p8_interval_sum_has_geometric_closed_form():
+    """Inside one control interval pitch is linear in n, so increments are geometric:
+    sum = inc_j * expm1(a R)/expm1(a), a = (pi_{j+1} - pi_j) ln2 / (12 R)."""
+    h = _swept_h()
+    sr, N = 8000, 500
+    E, L, M = O.controls(h, sr, N)
+    r = render_h(h, N, sr=sr, want_phase=True)
+    ph = np.unwrap(2 * np.pi * r["phase1"]) / (2 * np.pi)
+    for j in range(4):
+        pj = h[0] + h[68] + h[69] * M[0][j]; pj1 = h[0] + h[68] + h[69] * M[0][j + 1]
+        inc = 440.0 / sr * 2 ** ((pj - 69) / 12)
+        a = (pj1 - pj) * math.log(2) / 1200
+        s = inc * (math.expm1(100 * a) / math.expm1(a) if a else 100)
+        assert ph[100 * (j + 1)] - ph[100 * j] == pytest.approx(s, rel=1e-13)
+
+
+def test_p8_long_render_drift_bound_long_double():
+    """The oracle wraps phi every step; its own drift over 1.44 M samples at the most extreme pitch is
+    checked against an 80-bit long-double accumulation of the same increments (expect << 1e-6 cycles)."""
+    h = sine_only_h(midi=127.0)
+    h[68] = 24.0
+    N, sr = 1_440_000, 48000
+    r = render_h(h, N, sr=sr, want_phase=True)
+    inc = np.longdouble(440.0) / np.longdouble(sr) * np.exp2((np.longdouble(127.0 + 24.0) - 69) / 12)
+    for n in (1, 10**5, 10**6, N - 1):
+        want = float((np.longdouble(n) * inc) % 1)
+        d = abs(r["phase1"][n] - want)
+        assert min(d, 1 - d) < 1e-6
+
+
+# ----------------------------------------------------------------------------- P9 silence, mixer
+def test_p9_exact_silence_after_last_release():
+    u, nk = O.sample_params(0, 0, 16)
+    N = 4 * SR
+    for b in range(16):
+        r = O.render_voice(u[b], nk[b], SR, N, want_human=True)
+        h = r["human"]
+        t_end = h[1] + max(h[5], h[10], h[15], h[25])       # D + max release of adsr1, adsr2, lfo1_amp, lfo2_amp
+        n0 = 100 * (math.ceil(t_end * SR / 100) + 1)
+        if n0 < N:
+            assert np.all(r["audio"][n0:] == 0)
+            assert np.any(r["audio"][: n0] != 0)
+
+
+def test_p9_zero_levels_and_one_hot_mixer():
+    h = sine_only_h(); h[75] = 0.0
+    assert np.all(render_h(h, 500)["audio"] == 0)               # sum of levels 0 -> 0 (S13-14)
+    h = sine_only_h(); h[75] = 0.0; h[77] = 0.3; h[48 + 4 * 4 + 0] = 1.0   # noise only, a3 == 1
+    a = render_h(h, 400, noise_key=(7, 9))["audio"]
+    z = np.array([O.noise_value(O.noise_word(np.array([7, 9], dtype=np.uint32), n)) for n in range(400)])
+    assert np.allclose(a, z, atol=1e-16)                        # P11: noise-only voice = a3(n) z_n
+    h = sine_only_h(); h[75] = 0.2; h[76] = 0.6                 # vco2 level on but its amp row is 0
+    a = render_h(h, 400)["audio"]
+    assert np.allclose(a, 0.25 * np.sin(2 * np.pi * 440 * np.arange(400) / SR), atol=1e-13)
+
+
+def test_s13_vca_uses_upsampled_amp_row():
+    h = sine_only_h()
+    h[2:7] = [2000 / SR, 0, 1, 0, 1]                            # adsr1: linear attack ending ON tick 20
+    a = render_h(h, 4410)["audio"]
+    n = np.arange(4410)
+    env = np.minimum(n / 2000, 1.0)                              # piecewise linear with its kink on a tick
+                                                                 # => upsampling reproduces it (P7)
+    assert np.abs(a - env * np.sin(2 * np.pi * 440 * n / SR)).max() < 1e-12
+
+
+# ----------------------------------------------------------------------------- P10 squaresaw
+def test_p10_squaresaw_properties():
+    for k in (0.051, 3.0, 700.0, 18910.0):
+        for s in (0.0, 0.37, 1.0):
+            th = np.linspace(0.01, 6.27, 97)
+            y = np.array([O.squaresaw(t, k, s) for t in th])
+            ym = np.array([O.squaresaw(-t, k, s) for t in th])
+            assert np.allclose(y, -ym, atol=1e-15)                           # odd in theta
+            assert np.abs(y).max() <= 1.125 + 1e-12
+    assert O.squaresaw(1.0, 5000.0, 0.0) == pytest.approx(1.0, abs=1e-12)      # s = 0, large k: +-1
+    assert O.squaresaw(4.0, 5000.0, 0.0) == pytest.approx(-1.0, abs=1e-12)
+    assert O.squaresaw(0.7, 1e-4, 0.0) == pytest.approx(math.pi / 2 * 1e-4 * math.sin(0.7), rel=1e-6)
+    assert abs(O.squaresaw(math.pi, 50.0, 1.0)) < 1e-12                       # s = 1: zero at theta = pi
+    assert O.squaresaw(math.pi / 2, 1e6, 1.0) == pytest.approx(0.5, abs=1e-12)  # (1 - 1/2) * 1 * (1 + 0)
+    assert O.squaresaw(math.pi / 3, 1e6, 1.0) == pytest.approx(0.75, abs=1e-12)  # (1/2)(1 + cos 60deg)
+
+
+def test_s11_steepness_k_formula_and_range():
+    assert O.squaresaw_k(69.0, 0.0) == pytest.approx(12000 / (440 * math.log10(440)), rel=1e-15)
+    k_lo = O.squaresaw_k(127.0, 24.0); k_hi = O.squaresaw_k(0.0, -24.0)
+    assert k_lo == pytest.approx(0.051, abs=1e-3) and k_hi == pytest.approx(18910, rel=1e-3)
+
+
+def test_s11_vco2_in_voice_matches_formula():
+    h = neutral_h()
+    h[0], h[71], h[73], h[74] = 57.0, 3.0, 0.1, 0.6
+    h[48 + 4 * 3 + 0] = 1.0; h[76] = 1.0
+    N = 2000
+    a = render_h(h, N)["audio"]
+    fc = 440 * 2 ** ((57 + 3 - 69) / 12)
+    k = 12000 / (fc * math.log10(fc))
+    th = 2 * np.pi * (0.1 + fc * np.arange(N) / SR)
+    want = (1 - 0.3) * np.tanh(np.pi / 2 * k * np.sin(th)) * (1 + 0.6 * np.cos(th))
+    assert np.abs(a - want).max() < 1e-9
+
+
+# ----------------------------------------------------------------------------- P11 noise
+def test_p11_noise_moments_and_range():
+    key = np.array([0xdd2fc514, 0xadf5a0db], dtype=np.uint32)
+    z = np.array([O.noise_value(O.noise_word(key, n)) for n in range(40000)])
+    assert z.min() >= -1 and z.max() < 1
+    assert abs(z.mean()) < 4 * math.sqrt(1 / 3 / z.size)
+    assert abs(z.var() - 1 / 3) < 4 * math.sqrt(4 / 45 / z.size)
+    assert abs(np.corrcoef(z[:-1], z[1:])[0, 1]) < 0.03                     # white
+    assert O.noise_value(0) == -1.0 and O.noise_value(0xFFFFFFFF) == 1 - 2.0**-23
+    # word n is lane n&3 of Philox(key, (n>>2, 0, 0, 1)) (S12)
+    assert O.noise_word(key, 4 * 77 + 2) == py_philox([77, 0, 0, 1], [int(key[0]), int(key[1])])[2]
+
+
+# ----------------------------------------------------------------------------- P12 determinism / causality
+def test_p12_prefix_causality_and_determinism():
+    u, nk = O.sample_params(0, 0, 3)
+    for b in range(3):
+        a4 = O.render_voice(u[b], nk[b], SR, 4 * SR)["audio"]
+        a1 = O.render_voice(u[b], nk[b], SR, SR)["audio"]
+        assert np.array_equal(a1, a4[:SR])
+        assert np.array_equal(a1, O.render_voice(u[b], nk[b], SR, SR)["audio"])
+
+
+def test_d17_num_samples_and_ticks():
+    assert O.num_samples(44100, 4.0) == 176400 and O.num_samples(48000, 30) == 1440000   # 4 s
+    assert O.num_samples(44100, 0.00001) == 0 and O.num_samples(3, 0.5) == 2
+    assert O.num_ticks(176400) == 1765 and O.num_ticks(44100) == 442 and O.num_ticks(101) == 3 and O.num_ticks(1) == 2
+
+
+def test_p_paper_arithmetic_facts():
+    assert round(714e6 / 44100) == 16190                     # 714 MHz <=> ~16200 x real time
+    assert round(1e9 * 4 / 3600) == 1111111                  # 1 B x 4 s = 1,111,111 h
+
+
+# ----------------------------------------------------------------------------- whole voice (unpinned by the paper)
+def test_whole_voice_survey_probe_cross_check():
+    g = read_kv(os.path.join(GOLD, "survey_probe.txt"))
+    u, nk = O.sample_params(0, 0, 1)
+    r = O.render_voice(u[0], nk[0], SR, SR, want_human=True)
+    a, h = r["audio"], r["human"]
+    assert h[0] == pytest.approx(float(g["midi"]), abs=1e-6) and h[1] == pytest.approx(float(g["duration"]), abs=1e-6)
+    assert O.squaresaw_k(h[0], h[71]) == pytest.approx(float(g["k"]), abs=1e-6)
+    for n in (0, 1, 2, 1000, 22050, 44099):
+        assert a[n] == pytest.approx(float(g[f"out{n}"]), abs=1e-8)
+    assert math.sqrt(np.mean(a * a)) == pytest.approx(float(g["rms"]), abs=1e-8)
+    assert np.abs(a).max() == pytest.approx(float(g["max"]), abs=1e-8)
+
+
+def test_voice_independence_row_equals_single_render():
+    u, nk = O.sample_params(3, 2, 8)
+    batch = O.render_batch(u, nk, SR, 3000, threads=4)
+    for b in (0, 5, 7):
+        assert np.array_equal(batch[b], O.render_voice(u[b], nk[b], SR, 3000)["audio"])
