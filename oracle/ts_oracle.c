@@ -22,7 +22,8 @@
  *   sample_params ........ pinned: KAT-derived u[0..3] for (seed 0, g 0); layout by brute force
  *   map_param ............ pinned: closed forms (affine, end points, centre, inverse round trip)
  *   adsr ................. pinned: analytic segment-boundary values
- *   lfo / controls ....... pinned: closed forms with depth 0, one-hot shapes, table of shape values
+ *   lfo / controls ....... pinned: closed forms with depth 0, one-hot shapes, table of shape values,
+ *                          30 s phase against exact rational arithmetic (D21)
  *   upsample ............. pinned: linear signals reproduced, tick values hit
  *   vco phase / sine ..... pinned: sin(2*pi*f*t), exact 100-sample period, exact rational
  *                          cumulative sums on tiny inputs
@@ -229,7 +230,10 @@ void orc_controls(const double h[ORC_NPARAM], int sr, int64_t N, double *E_out, 
             double mix = (den == 0.0) ? 0.0 : num / den;
             L[l] = E[amp_e[l]] * mix;
             if (L_out) L_out[l * K + j] = L[l];
-            q[l] = q[l] + f / cr; /* exclusive sum: tick j used q_j */
+            /* exclusive sum: tick j used q_j.  Only frac(q) is ever read, so the running sum is kept
+             * mod 1 (reading D21), exactly as S9 does for the VCO phase: the wrap is exact and
+             * keeps this oracle's own rounding at ~1e-16 per tick instead of ulp(q) ~ 1e-13 at q ~ 900. */
+            q[l] = orc_frac(q[l] + f / cr);
         }
         const double src[4] = {E[0], E[1], L[0], L[1]};
         for (int d = 0; d < 5; ++d) {

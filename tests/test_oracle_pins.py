@@ -281,6 +281,25 @@ def test_p6_lfo_rate_and_amp_modulation_by_dedicated_adsrs():
     assert np.allclose(L[0][jj], amp * (2 * (q[jj] % 1.0) - 1), atol=1e-10)
 
 
+def test_d21_lfo_phase_30s_against_exact_rational_sum():
+    # D21: the LFO running sum is kept mod 1.  With depth = 0 the increment is the constant double
+    # delta = fl(f/cr); exact rational arithmetic gives p_j = frac(q0 + j*delta).  Read p back through a
+    # pure saw (2p - 1).  Measured: wrapped sum 1.7e-13 worst, unwrapped fp64 sum 5.7e-11 (q ~ 590, ulp 1.1e-13).
+    from fractions import Fraction
+    sr, N = 48000, 48000 * 30
+    cr = sr / 100
+    h = neutral_h(D=1000.0)
+    h[32], h[33], h[34] = 19.7, 0.0, -0.3125
+    h[35:40] = [0, 0, 1, 0, 0]
+    E, L, M = O.controls(h, sr, N)
+    delta = Fraction(19.7 / cr)
+    for j in list(range(0, 14401, 97)) + [14399, 14400]:
+        p = (Fraction(-0.3125) + j * delta) % 1
+        got = (L[0][j] + 1) / 2
+        d = abs(float(Fraction(got) - p))
+        assert min(d, 1 - d) < 1e-12, (j, d)
+
+
 def test_s7_modmix_weighted_mean():
     h = neutral_h()
     h[2:7] = [0, 0, 0.25, 0, 1]      # adsr1 == 0.25
