@@ -1,0 +1,113 @@
+/*
+ * tsynth.h -- C-ABI boundary of libtsynth.so: batched rendering of the default modular-synth Voice
+ * of arXiv 2104.12922 on one B200 (sm_100a).
+ *
+ * Citations: P:Lnnn = PAPER.md line nnn; S0..S14 / D1..D21 = the step definitions and readings listed
+ * in DESIGN.md ("Definition of the path", "Readings"), which restate SURVEY.md section 8(c).
+ *
+ * Conventions
+ *   - Every pointer is a DEVICE pointer unless its name starts with `host_` or the comment says host.
+ *   - The caller owns every buffer it passes in.  The library owns only an internal workspace
+ *     (control tables; grown on demand, released by ts_shutdown()).
+ *   - Calls enqueue work on the stream given to ts_set_stream() (default: the legacy stream 0) and
+ *     return without synchronising, except ts_render_host(), ts_sync() and ts_shutdown().
+ *   - Return value 0 = TS_OK, negative = error; ts_last_error() gives the text.  No exceptions,
+ *     no abort(), nothing printed.
+ *   - Not thread-safe: one host thread drives one library instance (one GPU per process).
+ */
+#ifndef TSYNTH_H
+#define TSYNTH_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TS_NPARAM 78 /* parameters of the default Voice */
+#define TS_R 100     /* audio rate / control rate, P:L117 (44.1 kHz / 441 Hz); reading D2 */
+
+enum {
+    TS_OK = 0,
+    TS_EINVAL = -1, /* B <= 0, sr <= 0, seconds <= 0, size overflow, nebula out of supported range */
+    TS_ENULL = -2,  /* a required pointer is NULL */
+    TS_ECUDA = -3,  /* a CUDA call failed; text in ts_last_error() */
+    TS_ENOMEM = -4  /* workspace allocation failed */
+};
+
+/* One voice's parameter record (320 B, 16-B aligned).  u[p] in [0,1] is the normalised parameter p
+ * ("sampled uniformly from the normalized range"), layout S2; noise_key seeds the voice's
+ * white-noise stream ("even of noise oscillators"; reading D4). */
+typedef struct {
+    float u[TS_NPARAM];
+    uint32_t noise_key[2];
+} ts_voice;
+
+/* One nebula entry: human range [lo, hi], curve exponent c (u^(1/c), reading D7),
+ * symmetric != 0 -> the curve acts on |2u-1| about the centre. */
+typedef struct {
+    double lo, hi, curve;
+    int64_t symmetric;
+} ts_range;
+
+typedef struct {
+    float *audio;        /* [B][N] row-major fp32, N = ts_num_samples(sr, seconds); required          */
+    float *params_human; /* [B][78] mapped parameter values (fp64 result rounded to fp32); may be NULL */
+} ts_out;
+
+/* S1 (readings D3, D5).  Voice b of the call is global voice g = batch_index*B + b.
+ * key = (seed lo32, seed hi32); Philox4x32-10 block i = 0..19 with counter (i, g lo32, g hi32, 0)
+ * gives words 4i..4i+3; u[p] = (word_p >> 8) * 2^-24; noise_key = first two words of the block with
+ * counter (0, g lo32, g hi32, 2).  Writes d_params[0..B).  Integer-exact; independent of B (D3). */
+int ts_sample_params(uint64_t seed, uint64_t batch_index, int B, ts_voice *d_params);
+
+/* S2..S14 (BASELINE.json north_star).  Renders B voices of `seconds` at `sr` Hz:
+ * parameter map -> 6 ADSR + 2 LFO at control ticks (every TS_R samples) -> modulation mixer ->
+ * linear upsampling -> phase-accumulating sine and square/saw VCOs + Philox white noise -> VCAs ->
+ * mixer -> out.audio.  u outside [0,1] (or NaN) is clamped to [0,1].  d_params is read only.
+ * Errors: TS_ENULL (d_params or out.audio NULL), TS_EINVAL (sizes; or the active nebula allows an
+ * oscillator increment beyond the supported 2^18/TS_R cycles per sample at this sr). */
+int ts_render(const ts_voice *d_params, int B, int sr, double seconds, ts_out out);
+
+/* Convenience end-to-end call with HOST buffers: ts_sample_params + ts_render on the device, then
+ * device->host copies of audio ([B][N] fp32) and, if host_params is not NULL, of the ts_voice
+ * records.  Synchronises.  Device staging memory belongs to the library workspace. */
+int ts_render_host(uint64_t seed, uint64_t batch_index, int B, int sr, double seconds,
+                   float *host_audio, ts_voice *host_params);
+
+/* D17: N = llround(sr*seconds);  S5: K = ceil(N/TS_R) + 1 control ticks. */
+int64_t ts_num_samples(int sr, double seconds);
+int64_t ts_num_ticks(int64_t N);
+
+int ts_set_stream(void *cuda_stream);              /* cudaStream_t; NULL = legacy default stream   */
+int ts_default_nebula(ts_range host_out78[TS_NPARAM]); /* host copy of the built-in table S2        */
+int ts_set_nebula(const ts_range *host_in78);      /* host table; NULL restores the default        */
+size_t ts_workspace_bytes(int B, int sr, double seconds); /* device bytes ts_render will hold      */
+const char *ts_last_error(void);                   /* host string, owned by the library            */
+int ts_sync(void);                                 /* cudaStreamSynchronize on the set stream      */
+void ts_shutdown(void);                            /* frees the workspace                          */
+
+/* Per-kernel device times of the LAST ts_render when timing is enabled (CUDA events on the set
+ * stream around each kernel; costs a few microseconds per call, so off by default).
+ * host_ms[0] = control kernel, host_ms[1] = audio kernel, summed over voice chunks; synchronises. */
+int ts_set_timing(int enable);
+int ts_last_kernel_ms(float host_ms[2]);
+/* Counters of the LAST ts_render (host): [0] kernels launched, [1] voice chunks,
+ * [2] audio samples in the active (non-silent) prefix summed over voices (valid after ts_sync). */
+int ts_last_stats(int64_t host_stats[3]);
+
+/* Debug exports used only by the parity tests. */
+/* S12: words n0..n0+count-1 of the noise stream of `key` (host array of 2) -> d_out[count]. */
+int ts_debug_noise_u32(const uint32_t host_key[2], uint64_t n0, int count, uint32_t *d_out);
+/* S5..S7: modulation-mixer rows at the control ticks -> d_ctl[B][5][K] fp64.  Rows 0 and 2 (pitch)
+ * are M_0, M_2; rows 1, 3, 4 are the amplitude rows M_1, M_3, M_4.  Ticks after the voice has gone
+ * silent for good (S4 release over on all four audible envelopes) are written as 0. */
+int ts_debug_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl);
+/* S9: phase of VCO `vco` (1 or 2) at every sample, cycles in [0,1) -> d_phase[B][N] fp64. */
+int ts_debug_phase(const ts_voice *d_params, int B, int sr, double seconds, int vco, double *d_phase);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TSYNTH_H */

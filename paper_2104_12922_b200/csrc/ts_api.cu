@@ -1,0 +1,347 @@
+// ts_api.cu -- the C-ABI of include/tsynth.h: argument checks, the nebula, the workspace (control tables
+// sized to stay L2-resident), voice chunking and kernel launches.  No arithmetic of the method lives here.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "ts_common.cuh"
+
+namespace {
+
+struct ts_state {
+    cudaStream_t stream = nullptr;
+    char err[512] = "";
+    ts_range nebula[TS_NPARAM];
+    bool nebula_init = false;
+    bool nebula_dirty = true;  // device constant copy is stale
+    // workspace
+    void *ws = nullptr;
+    size_t ws_bytes = 0;
+    // host staging for ts_render_host
+    void *stage = nullptr;
+    size_t stage_bytes = 0;
+    // timing / stats
+    bool timing = false;
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    float ms[2] = {0.f, 0.f};
+    int64_t stats[3] = {0, 0, 0};
+    unsigned long long *d_active = nullptr;
+    unsigned long long *h_active = nullptr;  // pinned
+};
+ts_state S;
+
+// Control-table budget per voice chunk: small enough to live in the 126 MB L2 next to the audio being
+// written, so the audio kernel's table reads never go to HBM.
+constexpr size_t TS_TABLE_BUDGET = 48u << 20;
+
+int fail(int code, const char *fmt, const char *detail = "") {
+    snprintf(S.err, sizeof S.err, fmt, detail);
+    return code;
+}
+int cuda_fail(cudaError_t e, const char *where) {
+    snprintf(S.err, sizeof S.err, "%s: %s", where, cudaGetErrorString(e));
+    return TS_ECUDA;
+}
+#define TS_CUDA(call)                                      \
+    do {                                                   \
+        cudaError_t e__ = (call);                          \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+    } while (0)
+
+void default_nebula(ts_range *n) {  // table S2 (D6, D8); ranges from BASELINE.json configs[0]
+    auto set = [&](int i, double lo, double hi, double c, int sym) { n[i] = ts_range{lo, hi, c, sym}; };
+    set(0, 0.0, 127.0, 1.0, 0);
+    set(1, 0.01, 1.0, 0.5, 0);
+    for (int e = 0; e < 6; ++e) {
+        const int b = 2 + 5 * e;
+        set(b + 0, 0.0, 2.0, 0.5, 0);
+        set(b + 1, 0.0, 2.0, 0.5, 0);
+        set(b + 2, 0.0, 1.0, 1.0, 0);
+        set(b + 3, 0.0, 2.0, 0.5, 0);
+        set(b + 4, 0.1, 6.0, 1.0, 0);
+    }
+    for (int l = 0; l < 2; ++l) {
+        const int b = 32 + 8 * l;
+        set(b + 0, 0.0, 20.0, 0.25, 0);
+        set(b + 1, -10.0, 10.0, 0.5, 1);
+        set(b + 2, -0.5, 0.5, 1.0, 0);
+        for (int i = 0; i < 5; ++i) set(b + 3 + i, 0.0, 1.0, 1.0, 0);
+    }
+    for (int i = 48; i < 68; ++i) set(i, 0.0, 1.0, 1.0, 0);
+    for (int v = 0; v < 2; ++v) {
+        const int b = 68 + 3 * v;
+        set(b + 0, -24.0, 24.0, 1.0, 1);
+        set(b + 1, -96.0, 96.0, 0.2, 1);
+        set(b + 2, -0.5, 0.5, 1.0, 0);
+    }
+    for (int i = 74; i < 78; ++i) set(i, 0.0, 1.0, 1.0, 0);
+}
+
+void ensure_nebula() {
+    if (!S.nebula_init) {
+        default_nebula(S.nebula);
+        S.nebula_init = true;
+        S.nebula_dirty = true;
+    }
+}
+
+// The audio kernel reads frac(phase) out of the fp64 mantissa after adding 1.5*2^19, which needs the
+// phase advance over one control interval to stay below 2^18 cycles (1.5*2^19 +- 2^18 keeps its exponent).
+bool nebula_supported(int sr) {
+    const ts_range *n = S.nebula;
+    auto hi = [&](int i) { return fmax(n[i].lo, n[i].hi); };
+    auto mag = [&](int i) { return fmax(fabs(n[i].lo), fabs(n[i].hi)); };
+    const double p1 = hi(0) + hi(68) + mag(69), p2 = hi(0) + hi(71) + mag(72);
+    const double inc = (440.0 / sr) * exp2((fmax(p1, p2) - 69.0) / 12.0);
+    return inc * TS_R < 262000.0;
+}
+
+int ensure_ws(size_t bytes) {
+    if (bytes <= S.ws_bytes) return TS_OK;
+    if (S.ws) cudaFree(S.ws);
+    S.ws = nullptr;
+    S.ws_bytes = 0;
+    if (cudaMalloc(&S.ws, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(TS_ENOMEM, "workspace allocation failed%s");
+    }
+    S.ws_bytes = bytes;
+    return TS_OK;
+}
+
+int chunk_voices(int B, int K) {
+    size_t per = (size_t)K * sizeof(ts_tick);
+    size_t c = TS_TABLE_BUDGET / per;
+    if (c < 1) c = 1;
+    if (c > (size_t)B) c = (size_t)B;
+    return (int)c;
+}
+size_t ws_layout(int Bc, int K, size_t *off_hdr) {
+    size_t table = ((size_t)Bc * K * sizeof(ts_tick) + 255) & ~(size_t)255;
+    if (off_hdr) *off_hdr = table;
+    return table + (((size_t)Bc * sizeof(ts_vhdr) + 255) & ~(size_t)255);
+}
+
+int check_sizes(int B, int sr, double seconds, int64_t *N, int *K) {
+    if (B <= 0 || sr <= 0 || !(seconds > 0.0)) return fail(TS_EINVAL, "B, sr and seconds must be positive%s");
+    const double ns = (double)sr * seconds;
+    if (!(ns < 2.0e9)) return fail(TS_EINVAL, "sr*seconds too large%s");
+    *N = ts_num_samples(sr, seconds);
+    if (*N <= 0) return fail(TS_EINVAL, "zero samples%s");
+    *K = (int)ts_num_ticks(*N);
+    if ((double)B * (double)*N > 9.0e18 / 8) return fail(TS_EINVAL, "B*N overflows%s");
+    return TS_OK;
+}
+
+int prepare_common(int sr) {
+    ensure_nebula();
+    if (!nebula_supported(sr)) return fail(TS_EINVAL, "nebula allows an oscillator increment above 2^18/R cycles per sample at this sr%s");
+    if (S.nebula_dirty) {
+        TS_CUDA(ts_upload_nebula(S.nebula, S.stream));
+        S.nebula_dirty = false;
+    }
+    if (!S.d_active) {
+        TS_CUDA(cudaMalloc(&S.d_active, sizeof(unsigned long long)));
+        TS_CUDA(cudaMallocHost(&S.h_active, sizeof(unsigned long long)));
+        *S.h_active = 0;
+    }
+    return TS_OK;
+}
+
+// mode 0: audio (+ optional params_human); 1/2: debug phase of VCO 1/2; 3: debug controls only
+int render_impl(const ts_voice *d_params, int B, int sr, double seconds, float *audio, float *params_human, int mode,
+                double *dbg) {
+    int64_t N;
+    int K;
+    int rc = check_sizes(B, sr, seconds, &N, &K);
+    if (rc) return rc;
+    rc = prepare_common(sr);
+    if (rc) return rc;
+    const int Bc = chunk_voices(B, K);
+    size_t off_hdr;
+    rc = ensure_ws(ws_layout(Bc, K, &off_hdr));
+    if (rc) return rc;
+    ts_tick *table = reinterpret_cast<ts_tick *>(S.ws);
+    ts_vhdr *hdr = reinterpret_cast<ts_vhdr *>(static_cast<char *>(S.ws) + off_hdr);
+
+    if (S.timing && mode == 0)
+        for (auto &e : S.ev)
+            if (!e) TS_CUDA(cudaEventCreate(&e));
+    S.ms[0] = S.ms[1] = 0.f;
+    int64_t launches = 0, chunks = 0;
+    TS_CUDA(cudaMemsetAsync(S.d_active, 0, sizeof(unsigned long long), S.stream));
+    if (mode == 3) TS_CUDA(cudaMemsetAsync(dbg, 0, (size_t)B * 5 * K * sizeof(double), S.stream));
+
+    for (int b0 = 0; b0 < B; b0 += Bc) {
+        const int nb = (B - b0 < Bc) ? (B - b0) : Bc;
+        const bool timed = S.timing && mode == 0;
+        if (timed) TS_CUDA(cudaEventRecord(S.ev[0], S.stream));
+        TS_CUDA(ts_launch_control(d_params + b0, nb, sr, N, K, table, hdr,
+                                  params_human ? params_human + (size_t)b0 * TS_NPARAM : nullptr,
+                                  mode == 3 ? dbg + (size_t)b0 * 5 * K : nullptr, S.d_active,
+                                  (mode == 1 || mode == 2) ? 1 : 0, S.stream));
+        ++launches;
+        if (timed) TS_CUDA(cudaEventRecord(S.ev[1], S.stream));
+        if (mode != 3) {
+            TS_CUDA(ts_launch_audio(table, hdr, nb, N, K, audio ? audio + (size_t)b0 * N : nullptr, mode,
+                                    (mode == 1 || mode == 2) ? dbg + (size_t)b0 * N : nullptr, S.stream));
+            ++launches;
+        }
+        if (timed) {
+            TS_CUDA(cudaEventRecord(S.ev[2], S.stream));
+            TS_CUDA(cudaEventSynchronize(S.ev[2]));
+            float a = 0.f, b = 0.f;
+            TS_CUDA(cudaEventElapsedTime(&a, S.ev[0], S.ev[1]));
+            TS_CUDA(cudaEventElapsedTime(&b, S.ev[1], S.ev[2]));
+            S.ms[0] += a;
+            S.ms[1] += b;
+        }
+        ++chunks;
+    }
+    TS_CUDA(cudaMemcpyAsync(S.h_active, S.d_active, sizeof(unsigned long long), cudaMemcpyDeviceToHost, S.stream));
+    S.stats[0] = launches;
+    S.stats[1] = chunks;
+    return TS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int64_t ts_num_samples(int sr, double seconds) { return (int64_t)llround((double)sr * seconds); }
+int64_t ts_num_ticks(int64_t N) { return (N + TS_R - 1) / TS_R + 1; }
+
+int ts_sample_params(uint64_t seed, uint64_t batch_index, int B, ts_voice *d_params) {
+    if (!d_params) return fail(TS_ENULL, "d_params is NULL%s");
+    if (B <= 0) return fail(TS_EINVAL, "B must be positive%s");
+    TS_CUDA(ts_launch_sample(seed, batch_index * (uint64_t)B, B, d_params, S.stream));
+    return TS_OK;
+}
+
+int ts_render(const ts_voice *d_params, int B, int sr, double seconds, ts_out out) {
+    if (!d_params) return fail(TS_ENULL, "d_params is NULL%s");
+    if (!out.audio) return fail(TS_ENULL, "out.audio is NULL%s");
+    return render_impl(d_params, B, sr, seconds, out.audio, out.params_human, 0, nullptr);
+}
+
+int ts_render_host(uint64_t seed, uint64_t batch_index, int B, int sr, double seconds, float *host_audio,
+                   ts_voice *host_params) {
+    if (!host_audio) return fail(TS_ENULL, "host_audio is NULL%s");
+    int64_t N;
+    int K;
+    int rc = check_sizes(B, sr, seconds, &N, &K);
+    if (rc) return rc;
+    const size_t pbytes = ((size_t)B * sizeof(ts_voice) + 255) & ~(size_t)255;
+    const size_t abytes = (size_t)B * N * sizeof(float);
+    if (pbytes + abytes > S.stage_bytes) {
+        if (S.stage) cudaFree(S.stage);
+        S.stage = nullptr;
+        S.stage_bytes = 0;
+        if (cudaMalloc(&S.stage, pbytes + abytes) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(TS_ENOMEM, "staging allocation failed%s");
+        }
+        S.stage_bytes = pbytes + abytes;
+    }
+    ts_voice *d_params = static_cast<ts_voice *>(S.stage);
+    float *d_audio = reinterpret_cast<float *>(static_cast<char *>(S.stage) + pbytes);
+    rc = ts_sample_params(seed, batch_index, B, d_params);
+    if (rc) return rc;
+    rc = render_impl(d_params, B, sr, seconds, d_audio, nullptr, 0, nullptr);
+    if (rc) return rc;
+    TS_CUDA(cudaMemcpyAsync(host_audio, d_audio, abytes, cudaMemcpyDeviceToHost, S.stream));
+    if (host_params)
+        TS_CUDA(cudaMemcpyAsync(host_params, d_params, (size_t)B * sizeof(ts_voice), cudaMemcpyDeviceToHost, S.stream));
+    TS_CUDA(cudaStreamSynchronize(S.stream));
+    return TS_OK;
+}
+
+int ts_set_stream(void *cuda_stream) {
+    S.stream = static_cast<cudaStream_t>(cuda_stream);
+    return TS_OK;
+}
+
+int ts_default_nebula(ts_range host_out78[TS_NPARAM]) {
+    if (!host_out78) return fail(TS_ENULL, "host_out78 is NULL%s");
+    default_nebula(host_out78);
+    return TS_OK;
+}
+
+int ts_set_nebula(const ts_range *host_in78) {
+    if (!host_in78) {
+        default_nebula(S.nebula);
+    } else {
+        for (int i = 0; i < TS_NPARAM; ++i) {
+            const ts_range &r = host_in78[i];
+            if (!(r.curve > 0.0) || !isfinite(r.lo) || !isfinite(r.hi) || !isfinite(r.curve))
+                return fail(TS_EINVAL, "nebula entries must be finite with curve > 0%s");
+        }
+        memcpy(S.nebula, host_in78, sizeof S.nebula);
+    }
+    S.nebula_init = true;
+    S.nebula_dirty = true;
+    return TS_OK;
+}
+
+size_t ts_workspace_bytes(int B, int sr, double seconds) {
+    int64_t N;
+    int K;
+    if (check_sizes(B, sr, seconds, &N, &K)) return 0;
+    return ws_layout(chunk_voices(B, K), K, nullptr);
+}
+
+const char *ts_last_error(void) { return S.err; }
+
+int ts_sync(void) {
+    TS_CUDA(cudaStreamSynchronize(S.stream));
+    if (S.h_active) S.stats[2] = (int64_t)*S.h_active;
+    return TS_OK;
+}
+
+void ts_shutdown(void) {
+    if (S.ws) cudaFree(S.ws);
+    if (S.stage) cudaFree(S.stage);
+    if (S.d_active) cudaFree(S.d_active);
+    if (S.h_active) cudaFreeHost(S.h_active);
+    for (auto &e : S.ev)
+        if (e) { cudaEventDestroy(e); e = nullptr; }
+    S.ws = S.stage = nullptr;
+    S.ws_bytes = S.stage_bytes = 0;
+    S.d_active = S.h_active = nullptr;
+    S.nebula_dirty = true;
+}
+
+int ts_set_timing(int enable) {
+    S.timing = enable != 0;
+    return TS_OK;
+}
+int ts_last_kernel_ms(float host_ms[2]) {
+    if (!host_ms) return fail(TS_ENULL, "host_ms is NULL%s");
+    host_ms[0] = S.ms[0];
+    host_ms[1] = S.ms[1];
+    return TS_OK;
+}
+int ts_last_stats(int64_t host_stats[3]) {
+    if (!host_stats) return fail(TS_ENULL, "host_stats is NULL%s");
+    if (S.h_active) S.stats[2] = (int64_t)*S.h_active;
+    memcpy(host_stats, S.stats, sizeof S.stats);
+    return TS_OK;
+}
+
+int ts_debug_noise_u32(const uint32_t host_key[2], uint64_t n0, int count, uint32_t *d_out) {
+    if (!host_key || !d_out) return fail(TS_ENULL, "NULL argument%s");
+    if (count <= 0) return fail(TS_EINVAL, "count must be positive%s");
+    TS_CUDA(ts_launch_noise_debug(host_key[0], host_key[1], n0, count, d_out, S.stream));
+    return TS_OK;
+}
+int ts_debug_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl) {
+    if (!d_params || !d_ctl) return fail(TS_ENULL, "NULL argument%s");
+    return render_impl(d_params, B, sr, seconds, nullptr, nullptr, 3, d_ctl);
+}
+int ts_debug_phase(const ts_voice *d_params, int B, int sr, double seconds, int vco, double *d_phase) {
+    if (!d_params || !d_phase) return fail(TS_ENULL, "NULL argument%s");
+    if (vco != 1 && vco != 2) return fail(TS_EINVAL, "vco must be 1 or 2%s");
+    return render_impl(d_params, B, sr, seconds, nullptr, nullptr, vco, d_phase);
+}
+
+}  // extern "C"

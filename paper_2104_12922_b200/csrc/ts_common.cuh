@@ -1,0 +1,70 @@
+// ts_common.cuh -- shared device-side definitions of libtsynth (CUDA path only; the CPU oracle
+// under oracle/ shares nothing with this file).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tsynth.h"
+
+// ---- geometry of the audio kernel --------------------------------------------------------------
+// One thread renders one RUN of consecutive samples; five runs make one control interval (TS_R).
+constexpr int TS_RUN = 20;                    // samples per thread (5 float4 groups, 5 Philox blocks)
+constexpr int TS_RUNS_PER_TICK = TS_R / TS_RUN;
+constexpr int TS_AUDIO_THREADS = 128;         // threads per CTA of the audio kernel
+constexpr int TS_TILE = TS_AUDIO_THREADS * TS_RUN;  // 2560 samples = 10 240 B staged in smem per CTA
+
+// ---- control table: one entry per control tick, written by the control kernel ------------------
+// phi  : VCO phase at the tick's first sample, cycles in [0,1)            (S9, exact integer scan)
+// inc  : phase increment of that sample, cycles/sample                    (S9)
+// e1   : rho - 1, rho = per-sample ratio of increments inside the interval (pitch is linear in n)
+// g20  : sum_{i<20} rho^i  (so that a run starting 20 samples later has phi += w*g20, w *= 1+e1*g20)
+// a1..a3 : VCA gains at the tick with the mixer level / level sum (and 1 - s/2 for VCO2) folded in
+struct __align__(16) ts_tick {
+    double phi1, inc1, e1_1, g20_1;
+    double phi2, inc2, e1_2, g20_2;
+    float a1, a2, a3, pad;
+};
+static_assert(sizeof(ts_tick) == 80, "ts_tick layout");
+
+// ---- per-voice header written by the control kernel -------------------------------------------
+struct __align__(16) ts_vhdr {
+    float shape;      // s of S11
+    float tanh_c;     // (pi/2) * k * 2*log2(e): tanh(x) = 1 - 2/(1 + 2^(tanh_c * sin(theta)))
+    uint32_t nk0, nk1;
+    int32_t n_act;    // samples [n_act, N) are exactly 0 (multiple of TS_R, or N)
+    int32_t n_ticks;  // table entries [0, n_ticks) are valid
+    int32_t pad[2];
+};
+static_assert(sizeof(ts_vhdr) == 32, "ts_vhdr layout");
+
+// ---- S0 Philox4x32-10 ---------------------------------------------------------------------------
+__device__ __forceinline__ void ts_philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                 uint32_t k0, uint32_t k1, uint32_t out[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        if (r > 0) {
+            k0 += 0x9E3779B9u;
+            k1 += 0xBB67AE85u;
+        }
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// launchers (host), one per .cu file
+cudaError_t ts_launch_sample(uint64_t seed, uint64_t g0, int B, ts_voice *d_params, cudaStream_t st);
+cudaError_t ts_launch_noise_debug(uint32_t k0, uint32_t k1, uint64_t n0, int count, uint32_t *d_out, cudaStream_t st);
+cudaError_t ts_upload_nebula(const ts_range *host78, cudaStream_t st);
+cudaError_t ts_launch_control(const ts_voice *d_params, int B, int sr, int64_t N, int K, ts_tick *table,
+                              ts_vhdr *hdr, float *params_human, double *dbg_ctl, unsigned long long *d_active,
+                              int full, cudaStream_t st);
+// mode 0: audio; mode 1 / 2: write the phase of VCO 1 / 2 (fp64 cycles) to dbg_phase instead
+cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, float *audio,
+                            int mode, double *dbg_phase, cudaStream_t st);

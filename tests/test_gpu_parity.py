@@ -1,0 +1,282 @@
+"""GPU parity tests: the CUDA path (through the C-ABI binding) against the fp64 CPU oracle, element by
+element on the same seeded inputs.  Bars (BASELINE.json north_star):
+  * bit-exact: every u (fp32 bit pattern), noise_key, raw Philox noise words;
+  * audio, per voice: max |g - o| <= 2e-3 AND relative RMS <= 1e-4, with reading D19 for silent voices.
+The oracle's inputs always come from the oracle's own sampler (never from the GPU).
+"""
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_2104_12922_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+MAX_ABS = 2e-3   # north_star
+REL_RMS = 1e-4   # north_star
+
+
+@pytest.fixture(scope="module")
+def T():
+    import torch
+    import paper_2104_12922_b200 as ts
+    assert torch.cuda.is_available()
+    ts.ts_set_nebula(None)
+    yield ts
+    ts.ts_set_nebula(None)
+
+
+def to_dev(u, nk):
+    import torch
+    rec = np.empty((u.shape[0], 80), dtype=np.float32)
+    rec[:, :78] = u
+    rec[:, 78:] = nk.view(np.float32)
+    return torch.from_numpy(rec).cuda()
+
+
+def voice_stats(g, o):
+    """g: fp32 GPU row, o: fp64 oracle row -> (max abs err, relative RMS err per D19)."""
+    d = g.astype(np.float64) - o
+    n = o.size
+    onorm = np.sqrt(np.sum(o * o))
+    rel = np.sqrt(np.sum(d * d)) / max(onorm, 1e-6 * np.sqrt(n))
+    return float(np.max(np.abs(d))) if n else 0.0, float(rel)
+
+
+def assert_parity(g, o, what=""):
+    worst = (0.0, 0.0, -1)
+    for b in range(o.shape[0]):
+        if not np.any(o[b]):
+            assert not np.any(g[b]), f"{what} voice {b}: oracle is exactly silent, GPU is not"
+            continue
+        mx, rel = voice_stats(g[b], o[b])
+        if mx > worst[0]:
+            worst = (mx, rel, b)
+        assert mx <= MAX_ABS and rel <= REL_RMS, f"{what} voice {b}: max|err|={mx:.3e} relRMS={rel:.3e}"
+    return worst
+
+
+def setup_workload(ts, name, batch_index=0, voices=None):
+    """-> (wl, nebula, u (edited, oracle-drawn), nk, device records built from the GPU's own draw)."""
+    wl = W.WORKLOADS[name]
+    u_o, nk_o = O.sample_params(wl.seed, batch_index, wl.B)
+    rec = ts.ts_sample_params(wl.seed, batch_index, wl.B).cpu().numpy()
+    assert np.array_equal(rec[:, :78].view(np.uint32), u_o.view(np.uint32)), "sampled u not bit-exact"
+    assert np.array_equal(rec[:, 78:].view(np.uint32), nk_o), "noise_key not bit-exact"
+    first = batch_index * wl.B
+    u = W.edit_u(u_o, wl, first)
+    u_g = W.edit_u(rec[:, :78], wl, first)
+    nk_g = np.ascontiguousarray(rec[:, 78:]).view(np.uint32)
+    if voices is not None:
+        u, nk_o, u_g, nk_g = u[voices], nk_o[voices], u_g[voices], nk_g[voices]
+    neb_o = W.apply_nebula(O.default_nebula(), wl)
+    ts.ts_set_nebula(W.apply_nebula(ts.ts_default_nebula(), wl))
+    return wl, neb_o, u, nk_o, to_dev(u_g, nk_g)
+
+
+# ---------------------------------------------------------------------------------- integers: bit-exact
+@pytest.mark.parametrize("seed,batch,B", [(0, 0, 4), (0, 0, 128), (7, 3, 128), (2**63 + 12345, 2**40, 1024),
+                                          (1, 2**32 - 1, 3), (0xFFFFFFFFFFFFFFFF, 0, 33)])
+def test_sampler_bit_exact(T, seed, batch, B):
+    rec = T.ts_sample_params(seed, batch, B).cpu().numpy()
+    u, nk = O.sample_params(seed, batch, B)
+    assert np.array_equal(rec[:, :78].view(np.uint32), u.view(np.uint32))
+    assert np.array_equal(rec[:, 78:].view(np.uint32), nk)
+
+
+def test_sampler_b_invariance(T):
+    a = T.ts_sample_params(5, 0, 256).cpu().numpy()
+    b = T.ts_sample_params(5, 1, 128).cpu().numpy()
+    assert np.array_equal(a[128:].view(np.uint32), b.view(np.uint32))
+
+
+@pytest.mark.parametrize("key,n0,count", [((0xdd2fc514, 0xadf5a0db), 0, 4096), ((1, 2), 176400 - 7, 1031),
+                                          ((0xFFFFFFFF, 0), 2**34 - 5, 64)])
+def test_noise_words_bit_exact(T, key, n0, count):
+    g = T.ts_debug_noise_u32(key, n0, count).cpu().numpy().view(np.uint32)
+    k = np.array(key, dtype=np.uint32)
+    o = np.array([O.noise_word(k, n0 + i) for i in range(count)], dtype=np.uint32)
+    assert np.array_equal(g, o)
+
+
+# ---------------------------------------------------------------------------------- control stage
+def test_controls_and_human_params_c1(T):
+    wl, neb, u, nk, dev = setup_workload(T, "C1")
+    ctl = T.ts_debug_controls(dev, wl.sr, wl.seconds).cpu().numpy()
+    _, human = T.ts_render(dev, wl.sr, wl.seconds, want_human=True)
+    human = human.cpu().numpy()
+    for b in range(wl.B):
+        h = O.map_all(u[b], neb)
+        assert np.allclose(human[b], h.astype(np.float32), rtol=2e-7, atol=0)
+        E, L, M = O.controls(h, wl.sr, wl.N)
+        assert np.max(np.abs(ctl[b] - M)) < 1e-12, b
+
+
+def test_phase_c1(T):
+    wl, neb, u, nk, dev = setup_workload(T, "C1")
+    for vco in (1, 2):
+        ph = T.ts_debug_phase(dev, wl.sr, wl.seconds, vco).cpu().numpy()
+        for b in range(wl.B):
+            r = O.render_voice(u[b], nk[b], wl.sr, wl.N, neb, want_phase=True)
+            d = np.abs(ph[b] - r[f"phase{vco}"])
+            d = np.minimum(d, 1 - d)
+            assert d.max() < 1e-9, (vco, b, d.max())
+
+
+# ---------------------------------------------------------------------------------- audio parity, all configs
+def test_audio_c1_every_sample(T):
+    wl, neb, u, nk, dev = setup_workload(T, "C1")
+    g = T.ts_render(dev, wl.sr, wl.seconds).cpu().numpy()
+    o = O.render_batch(u, nk, wl.sr, wl.N, neb)
+    print("C1 worst (max, relRMS, voice):", assert_parity(g, o, "C1"))
+
+
+def test_audio_c2_all_voices(T):
+    wl, neb, u, nk, dev = setup_workload(T, "C2")
+    g = T.ts_render(dev, wl.sr, wl.seconds).cpu().numpy()
+    o = O.render_batch(u, nk, wl.sr, wl.N, neb)
+    print("C2 worst (max, relRMS, voice):", assert_parity(g, o, "C2"))
+    # pin P9 on the GPU side: exact zeros wherever the oracle is exactly zero from some point on
+    for b in range(wl.B):
+        nzo = np.flatnonzero(o[b])
+        last = nzo[-1] + 1 if nzo.size else 0
+        assert not np.any(g[b, last:]), b
+
+
+@pytest.mark.parametrize("batch", [0, 49, 99])
+def test_audio_c3_batches_sampled_voices(T, batch):
+    voices = np.arange(0, 1024, 16)
+    wl, neb, u, nk, dev = setup_workload(T, "C3", batch_index=batch)
+    g = T.ts_render(dev, wl.sr, wl.seconds)[voices.tolist()].cpu().numpy()   # full-size launch, sampled rows
+    o = O.render_batch(u[voices], nk[voices], wl.sr, wl.N, neb)
+    print("C3 worst:", assert_parity(g, o, f"C3[{batch}]"))
+
+
+def test_audio_c4_long_render_all_voices(T):
+    wl, neb, u, nk, dev = setup_workload(T, "C4")
+    g = T.ts_render(dev, wl.sr, wl.seconds).cpu().numpy()
+    o = O.render_batch(u, nk, wl.sr, wl.N, neb)
+    print("C4 worst:", assert_parity(g, o, "C4"))
+    ph = T.ts_debug_phase(dev[:4].contiguous(), wl.sr, wl.seconds, 1).cpu().numpy()
+    for b in range(4):
+        r = O.render_voice(u[b], nk[b], wl.sr, wl.N, neb, want_phase=True)["phase1"]
+        for n in (0, 10**5, 10**6, wl.N - 1):
+            d = abs(ph[b, n] - r[n])
+            assert min(d, 1 - d) < 1e-7, (b, n, d)
+
+
+def test_audio_c5_full_launch_sampled_voices(T):
+    import torch
+    voices = np.concatenate([np.arange(0, 4096, 32), np.arange(1, 4096, 64)])
+    wl, neb, u, nk, dev = setup_workload(T, "C5")
+    full = T.ts_render(dev, wl.sr, wl.seconds)
+    g = full[torch.from_numpy(voices).cuda()].cpu().numpy()
+    del full
+    o = O.render_batch(u[voices], nk[voices], wl.sr, wl.N, neb)
+    print("C5 worst:", assert_parity(g, o, "C5"))
+
+
+# ---------------------------------------------------------------------------------- edge cases
+@pytest.mark.parametrize("sr,seconds,B", [(44100, 0.0123, 3), (44100, 0.00005, 2), (48000, 0.50001, 5),
+                                          (8000, 1.0, 2), (44100, 2560 / 44100, 1), (44101, 0.3, 2),
+                                          (96000, 0.25, 3)])
+def test_ragged_sizes(T, sr, seconds, B):
+    T.ts_set_nebula(None)
+    u, nk = O.sample_params(3, 1, B)
+    N = O.num_samples(sr, seconds)
+    assert T.ts_num_samples(sr, seconds) == N and T.ts_num_ticks(N) == O.num_ticks(N)
+    import torch
+    pad = torch.full((B * N + 64,), 7.0, device="cuda")       # guard words after the buffer
+    out = pad[:B * N].view(B, N)
+    T.ts_render(to_dev(u, nk), sr, seconds, out=out)
+    assert torch.all(pad[B * N:] == 7.0)
+    assert_parity(out.cpu().numpy(), O.render_batch(u, nk, sr, N), f"sr={sr} s={seconds}")
+
+
+def test_unaligned_output_pointer(T):
+    import torch
+    T.ts_set_nebula(None)
+    u, nk = O.sample_params(3, 2, 2)
+    sr, seconds = 44100, 0.2
+    N = O.num_samples(sr, seconds)
+    pad = torch.zeros(2 * N + 8, device="cuda")
+    out = pad[1:1 + 2 * N].view(2, N)                            # 4-byte aligned only
+    T.ts_render(to_dev(u, nk), sr, seconds, out=out)
+    assert_parity(out.cpu().numpy(), O.render_batch(u, nk, sr, N), "unaligned")
+
+
+def test_extreme_u_values(T):
+    T.ts_set_nebula(None)
+    rng = np.random.default_rng(11)
+    B = 24
+    u = rng.integers(0, 2, size=(B, 78)).astype(np.float32)     # every parameter at an end of its range
+    u[0] = 0.0
+    u[1] = 1.0
+    u[2] = 0.5
+    u[3, :] = np.float32(1) - np.float32(2.0**-24)
+    u[4, 75:78] = 0.0                                            # all mixer levels 0 -> exact silence
+    u[5, 48:68] = 0.0                                            # all mod weights 0 -> exact silence
+    # LFO rate / rate-depth / start phase stay generic: with end-of-range values (30 Hz at cr = 441 Hz, start
+    # phase 0.5) the phase lands EXACTLY on the square/saw jump every 147 ticks, where the sign is decided by
+    # the last rounding of either side (reading H8, "LFO tick flip"): not a well-posed parity input.
+    ur, _ = O.sample_params(11, 0, B)
+    for idx in (32, 33, 34, 40, 41, 42):
+        u[3:, idx] = ur[3:, idx]
+    nk = rng.integers(0, 2**32, size=(B, 2), dtype=np.uint64).astype(np.uint32)
+    sr, seconds = 44100, 1.5
+    N = O.num_samples(sr, seconds)
+    g = T.ts_render(to_dev(u, nk), sr, seconds).cpu().numpy()
+    o = O.render_batch(u, nk, sr, N)
+    assert_parity(g, o, "extreme u")
+    assert not np.any(g[4]) and not np.any(g[5])
+
+
+def test_out_of_range_u_is_clamped(T):
+    T.ts_set_nebula(None)
+    u, nk = O.sample_params(9, 0, 2)
+    u2 = u.copy()
+    u2[:, 5] = 1.5
+    u2[:, 9] = -0.25
+    u2[:, 12] = np.nan
+    sr, seconds = 44100, 0.5
+    g = T.ts_render(to_dev(u2, nk), sr, seconds).cpu().numpy()
+    o = O.render_batch(u2, nk, sr, O.num_samples(sr, seconds))
+    assert_parity(g, o, "clamp")
+
+
+def test_determinism_causality_independence(T):
+    import torch
+    wl, neb, u, nk, dev = setup_workload(T, "C1")
+    a = T.ts_render(dev, wl.sr, 1.0)
+    b = T.ts_render(dev, wl.sr, 1.0)
+    assert torch.equal(a, b)                                    # P12 bitwise determinism
+    c = T.ts_render(dev, wl.sr, 0.5)
+    assert torch.equal(c, a[:, :c.shape[1]])                    # P12 prefix / causality
+    d = T.ts_render(dev[2:3].contiguous(), wl.sr, 1.0)
+    assert torch.equal(d[0], a[2])                              # P3 voice independence
+
+
+def test_error_codes(T):
+    import torch
+    dev = T.ts_sample_params(0, 0, 2)
+    with pytest.raises(T.TsynthError):
+        T.ts_render(dev, 0, 1.0)
+    with pytest.raises(T.TsynthError):
+        T.ts_render(dev, 44100, -1.0)
+    neb = T.ts_default_nebula()
+    neb["hi"][0] = 400.0                                        # increment beyond the supported range
+    T.ts_set_nebula(neb)
+    with pytest.raises(T.TsynthError):
+        T.ts_render(dev, 44100, 0.1)
+    T.ts_set_nebula(None)
+    assert T.ts_render(dev, 44100, 0.1).shape == (2, 4410)
+    torch.cuda.synchronize()
+
+
+def test_render_host_end_to_end(T):
+    T.ts_set_nebula(None)
+    B, sr, seconds = 6, 44100, 0.75
+    N = O.num_samples(sr, seconds)
+    host = T.ts_render_host(4, 2, B, sr, seconds).numpy()
+    u, nk = O.sample_params(4, 2, B)
+    assert_parity(host, O.render_batch(u, nk, sr, N), "render_host")
