@@ -1,0 +1,271 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole hot path (sampler -> control -> audio) on synthetic workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl ours|reference]
+
+A step = one batch of the workload (BASELINE.json configs[1] = C2 by default: 128 voices x 4 s at 44.1 kHz)
+through ts_sample_params + ts_render, batch index = the step number (streaming corpus generation).
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "audio samples/sec"
+UNIT = "samples/s"
+FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(workload: str):
+    """dram bytes per launch of the audio kernel from the committed ncu --set full capture, if any."""
+    p = os.path.join(ROOT, "profiles", "audio_kernel_dram_bytes.json")
+    try:
+        with open(p) as f:
+            return json.load(f).get(workload)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """Polls NVML (the library behind nvidia-smi) for SM clock and throttle reasons while a region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _poll(self):
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def __enter__(self):
+        if self.nv:
+            self._thr = threading.Thread(target=self._poll, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+
+    def summary(self):
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_samples_per_s(wl, voices: int, repeats: int, threads: int):
+    import numpy as np
+    import oracle as O
+    from paper_2104_12922_b200 import workloads as W
+    O.build()
+    neb = W.apply_nebula(O.default_nebula(), wl)
+    u, nk = O.sample_params(wl.seed, 0, wl.B)
+    u = W.edit_u(u, wl)[:voices]
+    nk = nk[:voices]
+    O.render_batch(u[:1], nk[:1], wl.sr, min(wl.N, 4410), neb, threads=1)   # load the library
+    t0 = time.perf_counter()
+    for _ in range(repeats):
+        O.render_batch(u, nk, wl.sr, wl.N, neb, threads=threads, dtype=np.float32)
+    dt = time.perf_counter() - t0
+    return repeats * voices * wl.N / dt, dt
+
+
+def run_reference(args, wl):
+    """Base contract's reference arm for this tier: the oracle, as it stands, on the host cores."""
+    rank = int(os.environ.get("RANK", 0))
+    if rank != 0:
+        return
+    cores = os.cpu_count() or 1
+    voices = min(wl.B, 2 * cores)                 # bounded sample per step
+    for _ in range(args.warmup):
+        oracle_samples_per_s(wl, min(voices, cores), 1, cores)
+    t0 = time.perf_counter()
+    total = 0
+    for _ in range(args.steps):
+        v, _dt = oracle_samples_per_s(wl, voices, 1, cores)
+        total += voices * wl.N
+    dt = time.perf_counter() - t0
+    value = total / dt
+    sample = f"{voices} of {wl.B} voices x {wl.seconds} s per step, {cores} threads"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{wl.name}: B={wl.B} x {wl.seconds} s @ {wl.sr} Hz (oracle on a bounded sample: {sample})"},
+        "x_real_time": value / wl.sr,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_ours(args, wl):
+    import torch
+    import paper_2104_12922_b200 as ts
+    from paper_2104_12922_b200 import build, shard, workloads as W
+    build.build()
+    rank, local_rank, world = shard.init("nccl")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    B, sr, seconds, N = wl.B, wl.sr, wl.seconds, wl.N
+    ts.ts_set_nebula(W.apply_nebula(ts.ts_default_nebula(), wl))
+    if wl.edit != "none":
+        raise SystemExit("bench workloads with host-side parameter edits are parity-test cases (C4, C5): use C2 or C3")
+
+    # rotating output buffers: together larger than the 126 MB L2, so no step rewrites lines still cached
+    out_bytes = B * N * 4
+    nbuf = max(2, -(-(160 << 20) // out_bytes) + 1)
+    outs = [torch.empty((B, N), dtype=torch.float32, device=dev) for _ in range(nbuf)]
+    params = [torch.empty((B, 80), dtype=torch.float32, device=dev) for _ in range(nbuf)]
+
+    def step(i):
+        k = i % nbuf
+        ts.ts_sample_params(wl.seed, shard.batch_index(i, rank, world), B, out=params[k])
+        ts.ts_render(params[k], sr, seconds, out=outs[k])
+
+    for i in range(args.warmup):
+        step(i)
+    torch.cuda.synchronize()
+    shard.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clk:
+        torch.cuda.synchronize()
+        e0.record()
+        for i in range(args.steps):
+            step(args.warmup + i)
+        e1.record()
+        torch.cuda.synchronize()
+    shard.barrier()
+    ms = shard.max_over_ranks(e0.elapsed_time(e1), dev)
+    stats = ts.ts_last_stats()
+    launches_per_step = 1 + stats["launches"]
+    active_frac = stats["active_samples"] / float(B * N)
+    total_samples = float(B) * N * args.steps * world
+    value = total_samples / (ms * 1e-3)
+    clocks = clk.summary()
+    if clocks["samples"] < 5 and clk.nv:          # timed region too short for NVML: same load, untimed, 0.3 s
+        with ClockSampler(local_rank) as clk2:
+            t0 = time.perf_counter()
+            i = 0
+            while time.perf_counter() - t0 < 0.3:
+                step(i)
+                i += 1
+            torch.cuda.synchronize()
+        clocks = clk2.summary()
+        clocks["note"] = "timed region shorter than the NVML poll; sampled on the same loop run for 0.3 s"
+
+    # ---- roofline of the dominant kernel (audio): algorithmic bytes = 4 B per output sample
+    ts.ts_set_timing(True)
+    ctl_ms, aud_ms = [], []
+    for i in range(max(5, min(args.steps, 50))):
+        step(i)
+        c, a = ts.ts_last_kernel_ms()
+        ctl_ms.append(c)
+        aud_ms.append(a)
+    ts.ts_set_timing(False)
+    torch.cuda.synchronize()
+    aud = statistics.mean(aud_ms)
+    ctl = statistics.mean(ctl_ms)
+    peak, peak_src = measured_peak()
+    achieved = out_bytes / (aud * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "ts_audio_kernel<0>", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": ncu_traffic(wl.name), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": out_bytes, "audio_kernel_ms": aud, "control_kernel_ms": ctl,
+                "active_sample_fraction": active_frac,
+                "whole_step_frac_of_write_roofline": (4.0 * value / world / 1e9) / peak}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32 audio (f64 + Q0.64 integer phase chain)", "data": "synthetic",
+            "config": {"workload": f"{wl.name}: B={B} voices x {seconds} s @ {sr} Hz per GPU per step, seed 0, batch index = step",
+                       "l2": f"{nbuf} rotating output buffers of {out_bytes >> 20} MiB (> 126 MB L2 together)"},
+            "x_real_time": value / sr, "clocks": clocks, "gpu_launches": launches_per_step * args.steps,
+            "roofline": roofline,
+            "paper_context": "714e6 samples/s on one V100 (P:L23); other hardware, context only"}
+
+    # ---- end to end through the public host-buffer call: sample + render + D2H of audio and records
+    if rank == 0 or world > 1:
+        host = torch.empty((B, N), dtype=torch.float32, pin_memory=True)
+        hostp = torch.empty((B, 80), dtype=torch.float32, pin_memory=True)
+        n_e2e = max(3, min(args.steps, 10))
+        ts.ts_render_host(wl.seed, 0, B, sr, seconds, host, hostp)
+        shard.barrier()
+        t0 = time.perf_counter()
+        for i in range(n_e2e):
+            ts.ts_render_host(wl.seed, shard.batch_index(i, rank, world), B, sr, seconds, host, hostp)
+        dt = shard.max_over_ranks(time.perf_counter() - t0, dev)
+        line["e2e"] = {"value": float(B) * N * n_e2e * world / dt, "unit": UNIT, "h2d_bytes_per_step": 0,
+                       "d2h_bytes_per_step": out_bytes + B * 320, "steps": n_e2e,
+                       "note": "inputs are (seed, batch index) scalars: nothing to copy host->device"}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        v, dt = oracle_samples_per_s(wl, wl.B, 2, cores)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"all {wl.B} voices x {seconds} s, 2 repeats, {dt:.1f} s wall"}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    from paper_2104_12922_b200 import workloads as W
+    wl = W.WORKLOADS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, wl)
+    else:
+        run_ours(args, wl)
+
+
+if __name__ == "__main__":
+    main()

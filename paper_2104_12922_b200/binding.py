@@ -169,6 +169,8 @@ def ts_render(params, sr: int, seconds: float, out=None, want_human: bool = Fals
     torch = _torch()
     p = _dev_params(params)
     B = p.shape[0]
+    if ts_workspace_bytes(B, sr, float(seconds)) == 0:      # the library's own size check (TS_EINVAL)
+        raise TsynthError(f"libtsynth error -1: {lib().ts_last_error().decode()}")
     N = ts_num_samples(sr, seconds)
     if out is None:
         out = torch.empty((B, N), dtype=torch.float32, device=p.device)
