@@ -14,6 +14,8 @@ struct ts_state {
     ts_range nebula[TS_NPARAM];
     bool nebula_init = false;
     bool nebula_dirty = true;  // device constant copy is stale
+    bool math_uploaded = false;
+    unsigned int epoch = 0;    // look-back flag value of the latest control launch
     // workspace
     void *ws = nullptr;
     size_t ws_bytes = 0;
@@ -106,6 +108,9 @@ int ensure_ws(size_t bytes) {
         return fail(TS_ENOMEM, "workspace allocation failed%s");
     }
     S.ws_bytes = bytes;
+    // look-back flags must never equal a future epoch: start from zeros and restart the epoch count
+    if (cudaMemsetAsync(S.ws, 0, bytes, S.stream) != cudaSuccess) return cuda_fail(cudaGetLastError(), "cudaMemsetAsync");
+    S.epoch = 0;
     return TS_OK;
 }
 
@@ -116,10 +121,12 @@ int chunk_voices(int B, int K) {
     if (c > (size_t)B) c = (size_t)B;
     return (int)c;
 }
-size_t ws_layout(int Bc, int K, size_t *off_hdr) {
+size_t ws_layout(int Bc, int K, size_t *off_hdr, size_t *off_agg = nullptr) {
     size_t table = ((size_t)Bc * K * sizeof(ts_tick) + 255) & ~(size_t)255;
     if (off_hdr) *off_hdr = table;
-    return table + (((size_t)Bc * sizeof(ts_vhdr) + 255) & ~(size_t)255);
+    size_t agg = table + (((size_t)Bc * sizeof(ts_vhdr) + 255) & ~(size_t)255);
+    if (off_agg) *off_agg = agg;
+    return agg + ((ts_control_agg_bytes(Bc, K) + 255) & ~(size_t)255);
 }
 
 int check_sizes(int B, int sr, double seconds, int64_t *N, int *K) {
@@ -140,6 +147,10 @@ int prepare_common(int sr) {
         TS_CUDA(ts_upload_nebula(S.nebula, S.stream));
         S.nebula_dirty = false;
     }
+    if (!S.math_uploaded) {
+        TS_CUDA(ts_upload_math_tables(S.stream));
+        S.math_uploaded = true;
+    }
     if (!S.d_active) {
         TS_CUDA(cudaMalloc(&S.d_active, sizeof(unsigned long long)));
         TS_CUDA(cudaMallocHost(&S.h_active, sizeof(unsigned long long)));
@@ -158,11 +169,12 @@ int render_impl(const ts_voice *d_params, int B, int sr, double seconds, float *
     rc = prepare_common(sr);
     if (rc) return rc;
     const int Bc = chunk_voices(B, K);
-    size_t off_hdr;
-    rc = ensure_ws(ws_layout(Bc, K, &off_hdr));
+    size_t off_hdr, off_agg;
+    rc = ensure_ws(ws_layout(Bc, K, &off_hdr, &off_agg));
     if (rc) return rc;
     ts_tick *table = reinterpret_cast<ts_tick *>(S.ws);
     ts_vhdr *hdr = reinterpret_cast<ts_vhdr *>(static_cast<char *>(S.ws) + off_hdr);
+    void *agg = static_cast<char *>(S.ws) + off_agg;
 
     if (S.timing && mode == 0)
         for (auto &e : S.ev)
@@ -176,7 +188,11 @@ int render_impl(const ts_voice *d_params, int B, int sr, double seconds, float *
         const int nb = (B - b0 < Bc) ? (B - b0) : Bc;
         const bool timed = S.timing && mode == 0;
         if (timed) TS_CUDA(cudaEventRecord(S.ev[0], S.stream));
-        TS_CUDA(ts_launch_control(d_params + b0, nb, sr, N, K, table, hdr,
+        if (++S.epoch == 0) {  // wrapped after 2^32 launches: clear the flags and start over
+            TS_CUDA(cudaMemsetAsync(agg, 0, ts_control_agg_bytes(Bc, K), S.stream));
+            S.epoch = 1;
+        }
+        TS_CUDA(ts_launch_control(d_params + b0, nb, sr, N, K, table, hdr, agg, S.epoch,
                                   params_human ? params_human + (size_t)b0 * TS_NPARAM : nullptr,
                                   mode == 3 ? dbg + (size_t)b0 * 5 * K : nullptr, S.d_active,
                                   (mode == 1 || mode == 2) ? 1 : 0, S.stream));

@@ -62,9 +62,12 @@ __device__ __forceinline__ void ts_philox4x32_10(uint32_t c0, uint32_t c1, uint3
 cudaError_t ts_launch_sample(uint64_t seed, uint64_t g0, int B, ts_voice *d_params, cudaStream_t st);
 cudaError_t ts_launch_noise_debug(uint32_t k0, uint32_t k1, uint64_t n0, int count, uint32_t *d_out, cudaStream_t st);
 cudaError_t ts_upload_nebula(const ts_range *host78, cudaStream_t st);
+cudaError_t ts_upload_math_tables(cudaStream_t st);
+size_t ts_control_agg_bytes(int B, int K);  // look-back slots; must be zero before the first launch
+// epoch: a value never used before on this `agg` buffer (flags from older launches then read as "not ready")
 cudaError_t ts_launch_control(const ts_voice *d_params, int B, int sr, int64_t N, int K, ts_tick *table,
-                              ts_vhdr *hdr, float *params_human, double *dbg_ctl, unsigned long long *d_active,
-                              int full, cudaStream_t st);
+                              ts_vhdr *hdr, void *agg, unsigned int epoch, float *params_human, double *dbg_ctl,
+                              unsigned long long *d_active, int full, cudaStream_t st);
 // mode 0: audio; mode 1 / 2: write the phase of VCO 1 / 2 (fp64 cycles) to dbg_phase instead
 cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, float *audio,
                             int mode, double *dbg_phase, cudaStream_t st);

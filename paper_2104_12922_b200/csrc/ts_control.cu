@@ -1,62 +1,105 @@
 // ts_control.cu -- control-rate stage (S2..S7) and the tick-level phase scan of S9.
 //
-// One CTA per voice.  Per control tick j (tau_j = j*R/sr, S5) a thread evaluates the six ADSRs in
-// closed form (S4), the two LFOs (S6; each with its rate and amp ADSR) and the
-// modulation mixer (S7), all in fp64 because the two pitch rows feed the oscillator phase (H1 in
-// DESIGN.md).  The two running sums over time are done as block-wide prefix scans of Q0.64
-// fixed-point fractions of a cycle (warp __shfl_up_sync + per-warp totals + a carry between chunks of
-// blockDim ticks): integer addition mod 2^64 is exact and associative, so the scan order cannot change
-// a bit and phase does not drift however long the render is.
+// Flat grid over (voice, chunk of 127 control intervals); 128 threads, one control tick each (the last
+// thread's tick is the halo shared with the next chunk).  Per tick (tau_j = j*R/sr, S5) a thread evaluates
+// the six ADSRs in closed form (S4), the two LFOs (S6; each with its rate and amp ADSR,
+// P:L123) and the modulation mixer (S7), all in fp64 because the two pitch rows feed the oscillator phase
+// (H1 in DESIGN.md).  The two running sums over time are prefix scans of Q0.64 fixed-point fractions of a
+// cycle: __shfl_up_sync inside the warp, per-warp totals inside the CTA, and a decoupled look-back over the
+// chunk aggregates of the same voice (each CTA publishes its aggregate with an epoch flag and sums those
+// of its predecessors, which always have lower block indices).  Integer addition mod 2^64 is exact and
+// associative, so neither the scan order nor the look-back timing can change a bit, and phase does not
+// drift however long the render is.
 //   * LFO phase  q_j  = q_0 + sum_{i<j} f_i/cr                          (exclusive, mod 1; S6, D21)
 //   * VCO phase  Phi_j = phi_0 + sum_{i<j} S_i, S_i = sum of the R increments of interval i.
-//     Inside an interval pitch is linear in n (S8), so the increments are a geometric sequence and
-//     S_i = inc_i * expm1(R a)/expm1(a), a = (P_{i+1}-P_i) ln2 / (12 R)  (closed form; exact sum).
+//     Inside an interval pitch is linear in n (S8), so the increments are a geometric sequence:
+//     S_i = inc_i * (1 + rho + ... + rho^(R-1)), built by doubling (no division, no singularity at rho = 1).
 // The audio kernel then needs nothing from other threads: every run of 20 samples starts from the
 // table entry of its tick.
 #include "ts_common.cuh"
+#include "ts_math.cuh"
 
 __constant__ ts_range c_nebula[TS_NPARAM];
+__constant__ ts_math_tables c_math;
 
 cudaError_t ts_upload_nebula(const ts_range *host78, cudaStream_t st) {
     return cudaMemcpyToSymbolAsync(c_nebula, host78, sizeof(ts_range) * TS_NPARAM, 0, cudaMemcpyHostToDevice, st);
 }
 
+cudaError_t ts_upload_math_tables(cudaStream_t st) {
+    static ts_math_tables T;  // static: the async copy reads it after this function returns
+    for (int i = 0; i < TS_LOG_N; ++i) {
+        const unsigned long long lo = TS_LOG_OFF + ((unsigned long long)i << 47), hi = lo + (1ull << 47);
+        double zlo, zhi;
+        memcpy(&zlo, &lo, 8);
+        memcpy(&zhi, &hi, 8);
+        const long double c = ((long double)zlo + (long double)zhi) / 2.0L;
+        T.invc[i] = (double)(1.0L / c);
+        T.logc[i] = (double)(-log2l((long double)T.invc[i]));
+    }
+    for (int i = 0; i < TS_EXP_N; ++i) T.exp2t[i] = (double)exp2l((long double)i / TS_EXP_N);
+    return cudaMemcpyToSymbolAsync(c_math, &T, sizeof T, 0, cudaMemcpyHostToDevice, st);
+}
+
 // S3 map(u; lo,hi,c,S).  __dmul_rn/__dadd_rn: one rounding per operation (no FMA contraction), so the
 // affine parameters come out bit-identical to a plain IEEE evaluation of the same expression.
-__device__ double ts_map(double u, const ts_range &r) {
+__device__ __noinline__ double ts_pow_slow(double x, double a) { return pow(x, a); }  // cold paths only
+
+// x^a for x in [0,1], a > 0, exact at both ends
+__device__ __forceinline__ double ts_pow_unit(double x, double a, const ts_math_tables *T) {
+    if (x <= 0.0) return 0.0;
+    if (x >= 1.0) return 1.0;
+    return ts_pow01(x, a, T);
+}
+
+__device__ double ts_map(double u, const ts_range &r, const ts_math_tables *T) {
     if (!(u >= 0.0)) u = 0.0;
     if (u > 1.0) u = 1.0;
     if (!r.symmetric) {
-        const double v = (r.curve == 1.0) ? u : pow(u, 1.0 / r.curve);
+        const double v = (r.curve == 1.0) ? u : ts_pow_unit(u, 1.0 / r.curve, T);
         return __dadd_rn(r.lo, __dmul_rn(r.hi - r.lo, v));
     }
     const double d = __dadd_rn(__dmul_rn(2.0, u), -1.0);
     const double a = fabs(d);
-    const double v = (r.curve == 1.0) ? a : pow(a, 1.0 / r.curve);
+    const double v = (r.curve == 1.0) ? a : ts_pow_unit(a, 1.0 / r.curve, T);
     const double s = (d > 0.0) ? 1.0 : ((d < 0.0) ? -1.0 : 0.0);
     return __dadd_rn((r.lo + r.hi) / 2.0, __dmul_rn((r.hi - r.lo) / 2.0, s * v));
 }
 
+
+// ---- per-voice constants staged in shared memory by every CTA of the voice ---------------------------
+struct ts_voice_consts {
+    double h[TS_NPARAM + 2];  // mapped parameters (S2 layout)
+    double rs[18], rd[18], rinv[18];  // per ADSR the three ramps (release, attack, decay): start, duration, 1/duration
+    double lfo_w[2][5];       // LFO shape weights / their sum (0 if the sum is 0)
+    double mix_w[5][4];       // modulation-mixer weights / their row sum
+    double dq_f[2], dq_d[2];  // LFO frequency / cr and rate-mod depth / cr (cycles per tick)
+    double g[3];              // VCA gains: mixer level / level sum; VCO2 also carries (1 - s/2) of S11
+    int jsil;                 // first tick at which the voice is silent for good (== K if never)
+};
+
 // S4 ramp(t,s,d)^alpha.  pow(0,a) = 0 and pow(1,a) = 1 exactly for a > 0, so the saturated ends skip pow.
-__device__ __forceinline__ double ts_ramp_pow(double t, double s, double d, double alpha) {
+// The saturation tests are the oracle's own comparisons (exact); inside the ramp x/d is x * (1/d).
+__device__ __forceinline__ double ts_ramp_pow(double t, double s, double d, double invd, double alpha,
+                                              const ts_math_tables *T) {
     const double x = t - s;
-    double r;
-    if (x >= d) r = 1.0;
-    else if (x <= 0.0) r = 0.0;
-    else r = x / d;
-    if (alpha > 0.0 && (r == 0.0 || r == 1.0)) return r;
-    return pow(r, alpha);
+    if (!(alpha > 0.0)) return ts_pow_slow((x >= d) ? 1.0 : ((x <= 0.0) ? 0.0 : x / d), alpha);  // not with alpha > 0
+    if (x >= d) return 1.0;
+    if (x <= 0.0) return 0.0;
+    const double r = x * invd;
+    return (r >= 1.0) ? 1.0 : ts_pow01(r, alpha, T);
 }
 
-// E(t) = ramp(t,0,A)^a * [1 - (1-S) ramp(t,A,Dc)^a] * [1 - ramp(t,D,Rl)^a]
-__device__ __forceinline__ double ts_adsr(double t, const double *p, double D) {
-    const double A = p[0], Dc = p[1], S = p[2], Rl = p[3], al = p[4];
-    const double r = ts_ramp_pow(t, D, Rl, al);
+// E(t) = ramp(t,0,A)^a * [1 - (1-S) ramp(t,A,Dc)^a] * [1 - ramp(t,D,Rl)^a];  V ramps ordered release, attack, decay
+__device__ __forceinline__ double ts_adsr(double t, int e, const ts_voice_consts &V, const ts_math_tables *T) {
+    const double S = V.h[4 + 5 * e], al = V.h[6 + 5 * e];
+    const double *rs = &V.rs[3 * e], *rd = &V.rd[3 * e], *ri = &V.rinv[3 * e];
+    const double r = ts_ramp_pow(t, rs[0], rd[0], ri[0], al, T);
     if (r == 1.0) return 0.0;  // a * (...) * (1 - 1) = 0 exactly
-    const double a = ts_ramp_pow(t, 0.0, A, al);
+    const double a = ts_ramp_pow(t, rs[1], rd[1], ri[1], al, T);
     if (a == 0.0) return 0.0;
-    const double d = ts_ramp_pow(t, A, Dc, al);
-    return __dmul_rn(__dmul_rn(a, __dadd_rn(1.0, -__dmul_rn(1.0 - S, d))), 1.0 - r);
+    const double d = ts_ramp_pow(t, rs[2], rd[2], ri[2], al, T);
+    return a * (1.0 - (1.0 - S) * d) * (1.0 - r);
 }
 
 // frac of a double as Q0.64
@@ -68,10 +111,9 @@ __device__ __forceinline__ double ts_q64_to_double(unsigned long long q) {
     return __ull2double_rz(q >> 11) * (1.0 / 9007199254740992.0);  // exact truncation to 53 bits, [0,1)
 }
 
-// Block-wide exclusive scan (mod 2^64) of two values per thread, in thread order.  Returns the
-// exclusive prefix in (a, b) and the block totals in (ta, tb).  sm: 2*32 words of shared scratch.
-__device__ __forceinline__ void ts_block_scan2(unsigned long long &a, unsigned long long &b, unsigned long long &ta,
-                                               unsigned long long &tb, unsigned long long *sm) {
+// Block-wide exclusive scan (mod 2^64) of two values per thread, in thread order: __shfl_up_sync inside
+// the warp, per-warp totals through shared memory.  sm: 64 words of scratch.
+__device__ __forceinline__ void ts_block_scan2(unsigned long long &a, unsigned long long &b, unsigned long long *sm) {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
     unsigned long long ia = a, ib = b;
 #pragma unroll
@@ -82,75 +124,117 @@ __device__ __forceinline__ void ts_block_scan2(unsigned long long &a, unsigned l
     }
     if (lane == 31) { sm[wid] = ia; sm[32 + wid] = ib; }
     __syncthreads();
-    if (wid == 0) {
-        unsigned long long wa = (lane < nw) ? sm[lane] : 0ull, wb = (lane < nw) ? sm[32 + lane] : 0ull;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const unsigned long long ua = __shfl_up_sync(0xffffffffu, wa, o);
-            const unsigned long long ub = __shfl_up_sync(0xffffffffu, wb, o);
-            if (lane >= o) { wa += ua; wb += ub; }
-        }
-        sm[lane] = wa; sm[32 + lane] = wb;  // inclusive warp totals
-    }
-    __syncthreads();
-    const unsigned long long oa = wid ? sm[wid - 1] : 0ull, ob = wid ? sm[32 + wid - 1] : 0ull;
-    ta = sm[nw - 1]; tb = sm[32 + nw - 1];
+    unsigned long long oa = 0, ob = 0;
+    for (int w = 0; w < wid && w < nw; ++w) { oa += sm[w]; ob += sm[32 + w]; }  // <= 3 terms for 128 threads
     a = oa + ia - a;
     b = ob + ib - b;
     __syncthreads();  // scratch may be reused
 }
 
-// S6 LFO value at phase p in [0,1): normalised blend of the five shapes (D11).
-__device__ __forceinline__ double ts_lfo_mix(double p, const double *w) {
-    double sh[5];
-    sh[0] = sinpi(2.0 * p);
-    const double t = p + 0.75;
-    sh[1] = 4.0 * fabs((t - floor(t)) - 0.5) - 1.0;
-    sh[2] = 2.0 * p - 1.0;
-    sh[3] = 1.0 - 2.0 * p;
-    sh[4] = (p < 0.5) ? 1.0 : -1.0;
-    double num = 0.0, den = 0.0;
-#pragma unroll
-    for (int i = 0; i < 5; ++i) {
-        num = __dadd_rn(num, __dmul_rn(w[i], sh[i]));
-        den += w[i];
+// ---- decoupled look-back over the chunk aggregates of one voice ------------------------------------
+struct __align__(16) ts_agg {
+    unsigned long long s[2];
+    unsigned int flag;  // == launch epoch once s[] is valid
+    unsigned int pad[3];
+};
+static_assert(sizeof(ts_agg) == 32, "ts_agg layout");
+
+__device__ __forceinline__ void ts_publish(ts_agg *slot, unsigned long long a, unsigned long long b, unsigned int epoch) {
+    slot->s[0] = a;
+    slot->s[1] = b;
+    __threadfence();
+    *reinterpret_cast<volatile unsigned int *>(&slot->flag) = epoch;
+}
+// Threads 0..c-1 each fetch one predecessor's aggregate; the sums are combined through shared memory.
+__device__ __forceinline__ void ts_lookback(const ts_agg *slots, int c, unsigned int epoch, unsigned long long *acc /*smem[2]*/) {
+    for (int i = threadIdx.x; i < c; i += blockDim.x) {
+        const ts_agg *p = slots + i;
+        while (*reinterpret_cast<const volatile unsigned int *>(&p->flag) != epoch) __nanosleep(20);
+        __threadfence();
+        const unsigned long long a = *reinterpret_cast<const volatile unsigned long long *>(&p->s[0]);
+        const unsigned long long b = *reinterpret_cast<const volatile unsigned long long *>(&p->s[1]);
+        atomicAdd(&acc[0], a);
+        atomicAdd(&acc[1], b);
     }
-    return (den == 0.0) ? 0.0 : num / den;
 }
 
-struct ts_pitch2 {
-    double p1, p2;
-};
+// S6 LFO value at phase p in [0,1): blend of the five shapes with pre-normalised weights (D11).
+__device__ __forceinline__ double ts_lfo_mix(double p, const double *wn) {
+    const double t = p + 0.75;
+    double v = wn[0] * sinpi(2.0 * p);
+    v = fma(wn[1], 4.0 * fabs((t - floor(t)) - 0.5) - 1.0, v);
+    v = fma(wn[2], 2.0 * p - 1.0, v);
+    v = fma(wn[3], 1.0 - 2.0 * p, v);
+    v = fma(wn[4], (p < 0.5) ? 1.0 : -1.0, v);
+    return v;
+}
 
-__global__ void __launch_bounds__(1024)
-ts_control_kernel(const ts_voice *__restrict__ params, int sr, long long N, int K, ts_tick *__restrict__ table,
-                  ts_vhdr *__restrict__ hdr, float *__restrict__ params_human, double *__restrict__ dbg_ctl,
+constexpr int TS_CTL_THREADS = 128;
+constexpr int TS_CTL_IC = TS_CTL_THREADS - 1;  // control intervals per chunk (the last thread is the halo tick)
+
+__global__ void __launch_bounds__(TS_CTL_THREADS)
+ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long N, int K, int NC,
+                  ts_tick *__restrict__ table, ts_vhdr *__restrict__ hdr, ts_agg *__restrict__ agg,
+                  unsigned int epoch, float *__restrict__ params_human, double *__restrict__ dbg_ctl,
                   unsigned long long *__restrict__ d_active, int full) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double h[TS_NPARAM + 2];
+    __shared__ ts_voice_consts V;
+    __shared__ ts_math_tables MT;
     __shared__ unsigned long long scan_sm[64];
-    __shared__ int s_jsil;
-    ts_pitch2 *buf = reinterpret_cast<ts_pitch2 *>(smem_raw);  // [2][T + 1]
+    __shared__ unsigned long long acc[4];
+    __shared__ double2 pitch[TS_CTL_THREADS];
+    __shared__ double Es[6][TS_CTL_THREADS];
 
-    const int v = blockIdx.x, tid = threadIdx.x, T = blockDim.x;
+    const int tid = threadIdx.x;
+    const int c = blockIdx.x / B, v = blockIdx.x - c * B;  // chunk-major: predecessors have lower block indices
     const ts_voice &rec = params[v];
     ts_tick *tab = table + (size_t)v * K;
+    ts_agg *agg_q = agg + ((size_t)v * NC) * 2, *agg_p = agg_q + NC;
 
-    // ---- S2/S3: parameter map ----
+    // ---- stage tables, map the parameters (S2/S3), derive the per-voice constants ----
+    if (tid < (int)(sizeof(ts_math_tables) / 8))
+        reinterpret_cast<double *>(&MT)[tid] = reinterpret_cast<const double *>(&c_math)[tid];
+    if (tid < 4) acc[tid] = 0ull;
+    __syncthreads();
     if (tid < TS_NPARAM) {
-        const double hv = ts_map((double)rec.u[tid], c_nebula[tid]);
-        h[tid] = hv;
-        if (params_human) params_human[(size_t)v * TS_NPARAM + tid] = (float)hv;
+        const double hv = ts_map((double)rec.u[tid], c_nebula[tid], &MT);
+        V.h[tid] = hv;
+        if (params_human && c == 0) params_human[(size_t)v * TS_NPARAM + tid] = (float)hv;
     }
     __syncthreads();
-
+    const double *h = V.h;
     const double D = h[1];
     const double cr = (double)sr / (double)TS_R;
     const long long J = (N + TS_R - 1) / TS_R;  // control intervals that hold samples
-    // The voice is silent for good once the release of all four audible envelopes is over (their
-    // ramp is 1, so E = 0 exactly): adsr1, adsr2, lfo1_amp, lfo2_amp.
-    const double rl_max = fmax(fmax(h[2 + 3], h[7 + 3]), fmax(h[12 + 3], h[22 + 3]));
-    if (tid == 0) {
+    if (tid < 18) {  // ramps of ADSR e: release (starts at D), attack (0), decay (A)
+        const int e = tid / 3, k = tid - 3 * e;
+        const double A = h[2 + 5 * e], Dc = h[3 + 5 * e], Rl = h[5 + 5 * e];
+        const double st = (k == 0) ? D : ((k == 1) ? 0.0 : A), d = (k == 0) ? Rl : ((k == 1) ? A : Dc);
+        V.rs[tid] = st;
+        V.rd[tid] = d;
+        V.rinv[tid] = (d > 0.0) ? 1.0 / d : 0.0;
+    } else if (tid >= 32 && tid < 42) {
+        const int l = (tid - 32) / 5, i = (tid - 32) - 5 * l;
+        const double *w = &h[35 + 8 * l];
+        const double den = (((w[0] + w[1]) + w[2]) + w[3]) + w[4];
+        V.lfo_w[l][i] = (den == 0.0) ? 0.0 : w[i] / den;
+    } else if (tid >= 42 && tid < 46) {
+        const int l = (tid - 42) & 1;
+        if (tid < 44) V.dq_f[l] = h[32 + 8 * l] / cr;
+        else V.dq_d[l] = h[33 + 8 * l] / cr;
+    } else if (tid >= 64 && tid < 84) {
+        const int d = (tid - 64) >> 2, sidx = (tid - 64) & 3;
+        const double *w = &h[48 + 4 * d];
+        const double den = ((w[0] + w[1]) + w[2]) + w[3];
+        V.mix_w[d][sidx] = (den == 0.0) ? 0.0 : w[sidx] / den;
+    } else if (tid >= 97 && tid < 100) {
+        const int i = tid - 97;
+        const double lsum = (h[75] + h[76]) + h[77];
+        const double gi = (lsum == 0.0) ? 0.0 : h[75 + i] / lsum;
+        V.g[i] = (i == 1) ? gi * (1.0 - h[74] / 2.0) : gi;  // VCO2 carries (1 - s/2) of S11
+    } else if (tid == 96) {
+        // The voice is silent for good once the release of all four audible envelopes is over (their
+        // ramp is 1, so E = 0 exactly): adsr1, adsr2, lfo1_amp, lfo2_amp.
+        const double rl_max = fmax(fmax(h[2 + 3], h[7 + 3]), fmax(h[12 + 3], h[22 + 3]));
         long long j = (long long)floor((D + rl_max) * cr) - 2;
         if (j < 0) j = 0;
         if (j > K - 1) j = K - 1;
@@ -158,147 +242,132 @@ ts_control_kernel(const ts_voice *__restrict__ params, int sr, long long N, int 
         while (j < K && !(((double)(j * TS_R) / (double)sr) - D >= rl_max)) ++j;
         while (j > 0 && (((double)((j - 1) * TS_R) / (double)sr) - D >= rl_max)) --j;
         if (full) j = K;  // debug exports: evaluate every tick
-        s_jsil = (int)j;  // == K if never silent inside the table
-        const long long n_act = (j * TS_R < N) ? j * TS_R : N;
-        ts_vhdr hd;
-        hd.shape = (float)h[74];
-        const double fc = 440.0 * exp2((h[0] + h[71] - 69.0) / 12.0);
-        const double k = 12000.0 / (fc * log10(fc));
-        hd.tanh_c = (float)(1.5707963267948966 * k * 2.0 * 1.4426950408889634);
-        hd.nk0 = rec.noise_key[0];
-        hd.nk1 = rec.noise_key[1];
-        hd.n_act = (int32_t)n_act;
-        hd.n_ticks = (int32_t)((j + 1 < K) ? j + 1 : K);
-        hd.pad[0] = hd.pad[1] = 0;
-        hdr[v] = hd;
-        if (d_active) atomicAdd(d_active, (unsigned long long)n_act);
+        V.jsil = (int)j;
+        if (c == 0) {
+            const long long n_act = (j * TS_R < N) ? j * TS_R : N;
+            ts_vhdr hd;
+            hd.shape = (float)h[74];
+            const double fc = 440.0 * ts_exp2((h[0] + h[71] - 69.0) * (1.0 / 12.0), &MT);
+            const double k = 12000.0 / (fc * (ts_log2(fc, &MT) * 0.30102999566398120));
+            hd.tanh_c = (float)(1.5707963267948966 * k * 2.0 * 1.4426950408889634);
+            hd.nk0 = rec.noise_key[0];
+            hd.nk1 = rec.noise_key[1];
+            hd.n_act = (int32_t)n_act;
+            hd.n_ticks = (int32_t)((j + 1 < K) ? j + 1 : K);
+            hd.pad[0] = hd.pad[1] = 0;
+            hdr[v] = hd;
+            if (d_active) atomicAdd(d_active, (unsigned long long)n_act);
+        }
     }
     __syncthreads();
-    const int jsil = s_jsil;
-    const int n_ticks = (jsil + 1 < K) ? jsil + 1 : K;
+    const int jsil = V.jsil;
+    const int j0 = c * TS_CTL_IC;
+    if (c > 0 && j0 >= jsil) return;  // nothing audible from this chunk on; no successor waits for it
 
-    // mixer gains folded into the amp rows (S13/S14): l_i / (l1+l2+l3); VCO2 also carries (1 - s/2) of S11
-    const double lsum = (h[75] + h[76]) + h[77];
-    const double g1 = (lsum == 0.0) ? 0.0 : h[75] / lsum;
-    const double g2 = (lsum == 0.0) ? 0.0 : h[76] / lsum * (1.0 - h[74] / 2.0);
-    const double g3 = (lsum == 0.0) ? 0.0 : h[77] / lsum;
-    const double base1 = h[0] + h[68], base2 = h[0] + h[71];
-    const double dep1 = h[69], dep2 = h[72];
-    const double f0 = 440.0 / (double)sr;
-
-    unsigned long long carry_q1 = ts_frac_q64(h[34]), carry_q2 = ts_frac_q64(h[42]);
-    unsigned long long carry_p1 = ts_frac_q64(h[70]), carry_p2 = ts_frac_q64(h[73]);
-
-    const int nch = (n_ticks + T - 1) / T;
-    for (int c = 0; c <= nch; ++c) {
-        // ================= phase 1: controls at tick j =================
-        const int j = c * T + tid;
-        const bool live = (c < nch) && (j < n_ticks);
-        double E[6] = {0, 0, 0, 0, 0, 0};
-        unsigned long long dq1 = 0, dq2 = 0;
-        if (live) {
-            const double tau = (double)((long long)j * TS_R) / (double)sr;
+    // ================= phase 1: controls at tick j =================
+    const int j = j0 + tid;
+    const bool live = (j <= jsil) && (j < K);
+    double E[6] = {0, 0, 0, 0, 0, 0};
+    unsigned long long dq1 = 0, dq2 = 0;
+    if (live) {
+        const double tau = (double)((long long)j * TS_R) / (double)sr;
+#pragma unroll 1
+        for (int e = 0; e < 6; ++e) Es[e][tid] = ts_adsr(tau, e, V, &MT);  // rolled: one copy of the pow code
 #pragma unroll
-            for (int e = 0; e < 6; ++e) E[e] = ts_adsr(tau, &h[2 + 5 * e], D);
-            const double d1 = __dadd_rn(h[32], __dmul_rn(h[33], E[3])) / cr;
-            const double d2 = __dadd_rn(h[40], __dmul_rn(h[41], E[5])) / cr;
-            dq1 = (unsigned long long)__double2ll_rn((d1 - rint(d1)) * 18446744073709551616.0);
-            dq2 = (unsigned long long)__double2ll_rn((d2 - rint(d2)) * 18446744073709551616.0);
-        }
-        if (c < nch) {
-            unsigned long long t1, t2;
-            ts_block_scan2(dq1, dq2, t1, t2, scan_sm);
-            const unsigned long long q1 = carry_q1 + dq1, q2 = carry_q2 + dq2;
-            carry_q1 += t1;
-            carry_q2 += t2;
-            if (live) {
-                const double L1 = __dmul_rn(E[2], ts_lfo_mix(ts_q64_to_double(q1), &h[35]));
-                const double L2 = __dmul_rn(E[4], ts_lfo_mix(ts_q64_to_double(q2), &h[43]));
-                const double src[4] = {E[0], E[1], L1, L2};
-                double M[5];
+        for (int e = 0; e < 6; ++e) E[e] = Es[e][tid];
+        const double d1 = fma(V.dq_d[0], E[3], V.dq_f[0]);
+        const double d2 = fma(V.dq_d[1], E[5], V.dq_f[1]);
+        dq1 = (unsigned long long)__double2ll_rn((d1 - rint(d1)) * 18446744073709551616.0);
+        dq2 = (unsigned long long)__double2ll_rn((d2 - rint(d2)) * 18446744073709551616.0);
+    }
+    ts_block_scan2(dq1, dq2, scan_sm);  // exclusive prefix inside the chunk
+    if (tid == TS_CTL_IC) ts_publish(&agg_q[c], dq1, dq2, epoch);  // halo thread: sum over the chunk's own 127 ticks
+    ts_lookback(agg_q, c, epoch, &acc[0]);
+    __syncthreads();
+    const unsigned long long q1 = ts_frac_q64(h[34]) + acc[0] + dq1, q2 = ts_frac_q64(h[42]) + acc[1] + dq2;
+    if (live) {
+#pragma unroll 1
+        for (int l = 0; l < 2; ++l)  // rolled: one copy of the sinpi code
+            Es[l][tid] = Es[2 + 2 * l][tid] * ts_lfo_mix(ts_q64_to_double(l ? q2 : q1), V.lfo_w[l]);
+        const double L1 = Es[0][tid], L2 = Es[1][tid];
+        double M[5];
 #pragma unroll
-                for (int d = 0; d < 5; ++d) {
-                    double num = 0.0, den = 0.0;
+        for (int d = 0; d < 5; ++d)
+            M[d] = fma(V.mix_w[d][3], L2, fma(V.mix_w[d][2], L1, fma(V.mix_w[d][1], E[1], V.mix_w[d][0] * E[0])));
+        pitch[tid] = make_double2(fma(h[69], M[0], h[0] + h[68]), fma(h[72], M[2], h[0] + h[71]));
+        // the halo tick is written by the next chunk unless that chunk has nothing to do
+        if (tid < TS_CTL_IC || j0 + TS_CTL_IC >= jsil) {
+            float4 a;
+            a.x = (float)(M[1] * V.g[0]);
+            a.y = (float)(M[3] * V.g[1]);
+            a.z = (float)(M[4] * V.g[2]);
+            a.w = 0.0f;
+            *reinterpret_cast<float4 *>(&tab[j].a1) = a;
+            if (dbg_ctl) {
+                double *o = dbg_ctl + (size_t)v * 5 * K;
 #pragma unroll
-                    for (int s = 0; s < 4; ++s) {
-                        num = __dadd_rn(num, __dmul_rn(h[48 + 4 * d + s], src[s]));
-                        den += h[48 + 4 * d + s];
-                    }
-                    M[d] = (den == 0.0) ? 0.0 : num / den;
-                }
-                ts_pitch2 pp;
-                pp.p1 = __dadd_rn(base1, __dmul_rn(dep1, M[0]));
-                pp.p2 = __dadd_rn(base2, __dmul_rn(dep2, M[2]));
-                buf[(c & 1) * (T + 1) + tid] = pp;
-                float4 a;
-                a.x = (float)(M[1] * g1);
-                a.y = (float)(M[3] * g2);
-                a.z = (float)(M[4] * g3);
-                a.w = 0.0f;
-                *reinterpret_cast<float4 *>(&tab[j].a1) = a;
-                if (dbg_ctl) {
-                    double *o = dbg_ctl + (size_t)v * 5 * K;
-#pragma unroll
-                    for (int d = 0; d < 5; ++d) o[(size_t)d * K + j] = M[d];
-                }
+                for (int d = 0; d < 5; ++d) o[(size_t)d * K + j] = M[d];
             }
         }
-        __syncthreads();
-        // ================= phase 2: interval jj = (c-1)*T + tid =================
-        if (c > 0) {
-            const int jj = (c - 1) * T + tid;
-            const bool act = (jj + 1 < n_ticks) && (jj < J);
-            unsigned long long s1 = 0, s2 = 0;
-            double inc1 = 0, inc2 = 0, e1a = 0, e1b = 0, g20a = TS_RUN, g20b = TS_RUN;
-            if (act) {
-                const ts_pitch2 p0 = buf[((c - 1) & 1) * (T + 1) + tid];
-                const ts_pitch2 p1 = (tid + 1 < T) ? buf[((c - 1) & 1) * (T + 1) + tid + 1] : buf[(c & 1) * (T + 1)];
-                {
-                    inc1 = f0 * exp2((p0.p1 - 69.0) / 12.0);
-                    const double a = (p1.p1 - p0.p1) * (0.69314718055994530942 / (12.0 * TS_R));
-                    e1a = expm1(a);
-                    const double e20 = expm1(TS_RUN * a);
-                    const double e40 = e20 * (2.0 + e20), e80 = e40 * (2.0 + e40);
-                    const double e100 = e80 + e20 + e80 * e20;
-                    g20a = (e1a == 0.0) ? (double)TS_RUN : e20 / e1a;
-                    s1 = ts_frac_q64(inc1 * ((e1a == 0.0) ? (double)TS_R : e100 / e1a));
-                }
-                {
-                    inc2 = f0 * exp2((p0.p2 - 69.0) / 12.0);
-                    const double a = (p1.p2 - p0.p2) * (0.69314718055994530942 / (12.0 * TS_R));
-                    e1b = expm1(a);
-                    const double e20 = expm1(TS_RUN * a);
-                    const double e40 = e20 * (2.0 + e20), e80 = e40 * (2.0 + e40);
-                    const double e100 = e80 + e20 + e80 * e20;
-                    g20b = (e1b == 0.0) ? (double)TS_RUN : e20 / e1b;
-                    s2 = ts_frac_q64(inc2 * ((e1b == 0.0) ? (double)TS_R : e100 / e1b));
-                }
-            }
-            unsigned long long t1, t2;
-            ts_block_scan2(s1, s2, t1, t2, scan_sm);
-            const unsigned long long P1 = carry_p1 + s1, P2 = carry_p2 + s2;
-            carry_p1 += t1;
-            carry_p2 += t2;
-            if (act) {
-                double4 *dst = reinterpret_cast<double4 *>(&tab[jj]);
-                // 16-byte stores (double2) keep the table writes vectorised without 32-byte alignment
-                double2 *d2 = reinterpret_cast<double2 *>(dst);
-                d2[0] = make_double2(ts_q64_to_double(P1), inc1);
-                d2[1] = make_double2(e1a, g20a);
-                d2[2] = make_double2(ts_q64_to_double(P2), inc2);
-                d2[3] = make_double2(e1b, g20b);
-            }
+    }
+    __syncthreads();
+
+    // ================= phase 2: interval j (pitch is linear between ticks j and j+1) =================
+    const bool act = (tid < TS_CTL_IC) && (j < jsil) && (j < J);
+    unsigned long long s1 = 0, s2 = 0;
+    double inc[2] = {0, 0}, e1[2] = {0, 0}, g20[2] = {TS_RUN, TS_RUN};
+    if (act) {
+        const double2 p0 = pitch[tid], p1 = pitch[tid + 1];
+        const double f0 = 440.0 / (double)sr;
+#pragma unroll 1
+        for (int o = 0; o < 2; ++o) {
+            const double pa = o ? p0.y : p0.x, pb = o ? p1.y : p1.x;
+            const double inc0_ = f0 * ts_exp2((pa - 69.0) * (1.0 / 12.0), &MT);
+            const double x1 = ts_expm1_small((pb - pa) * (0.69314718055994530942 / (12.0 * TS_R)));  // rho - 1
+            // geometric sums by doubling: x_m = rho^m - 1, g_m = 1 + rho + ... + rho^(m-1)
+            const double x2 = x1 * (2.0 + x1), x4 = x2 * (2.0 + x2);
+            const double g2 = 2.0 + x1, g4 = g2 * (2.0 + x2);
+            const double g5 = g4 + (1.0 + x4), x5 = fma(x4, x1, x4 + x1);
+            const double g10 = g5 * (2.0 + x5), x10 = x5 * (2.0 + x5);
+            const double g20_ = g10 * (2.0 + x10), x20 = x10 * (2.0 + x10);
+            const double g40 = g20_ * (2.0 + x20), x40 = x20 * (2.0 + x20);
+            const double g80 = g40 * (2.0 + x40), x80 = x40 * (2.0 + x40);
+            const double g100 = fma(1.0 + x80, g20_, g80);
+            const double inc_ = inc0_;
+            const unsigned long long sf = ts_frac_q64(inc_ * g100);
+            if (o) { s2 = sf; inc[1] = inc_; e1[1] = x1; g20[1] = g20_; }
+            else   { s1 = sf; inc[0] = inc_; e1[0] = x1; g20[0] = g20_; }
         }
-        // buf[(c-1)&1] is rewritten in iteration c+1's phase 1, after the barriers inside this iteration's scan
+    }
+    ts_block_scan2(s1, s2, scan_sm);
+    if (tid == TS_CTL_IC) ts_publish(&agg_p[c], s1, s2, epoch);
+    ts_lookback(agg_p, c, epoch, &acc[2]);
+    __syncthreads();
+    if (act) {
+        const unsigned long long P1 = ts_frac_q64(h[70]) + acc[2] + s1, P2 = ts_frac_q64(h[73]) + acc[3] + s2;
+        double2 *d2 = reinterpret_cast<double2 *>(&tab[j]);
+        d2[0] = make_double2(ts_q64_to_double(P1), inc[0]);
+        d2[1] = make_double2(e1[0], g20[0]);
+        d2[2] = make_double2(ts_q64_to_double(P2), inc[1]);
+        d2[3] = make_double2(e1[1], g20[1]);
     }
 }
 
+size_t ts_control_agg_bytes(int B, int K) {
+    const int J = K - 1, NC = (J + TS_CTL_IC - 1) / TS_CTL_IC > 0 ? (J + TS_CTL_IC - 1) / TS_CTL_IC : 1;
+    return (size_t)B * NC * 2 * sizeof(ts_agg);
+}
+
 cudaError_t ts_launch_control(const ts_voice *d_params, int B, int sr, int64_t N, int K, ts_tick *table,
-                              ts_vhdr *hdr, float *params_human, double *dbg_ctl, unsigned long long *d_active,
-                              int full, cudaStream_t st) {
-    // few voices: one big CTA per voice (the chip is otherwise idle); many voices: smaller CTAs, several per SM
-    const int T = (B <= 296) ? 1024 : 256;
-    const size_t smem = 2 * (size_t)(T + 1) * sizeof(ts_pitch2);
-    ts_control_kernel<<<B, T, smem, st>>>(d_params, sr, (long long)N, K, table, hdr, params_human, dbg_ctl, d_active, full);
+                              ts_vhdr *hdr, void *agg, unsigned int epoch, float *params_human, double *dbg_ctl,
+                              unsigned long long *d_active, int full, cudaStream_t st) {
+    const int J = K - 1;
+    int NC = (J + TS_CTL_IC - 1) / TS_CTL_IC;
+    if (NC < 1) NC = 1;
+    const long long grid = (long long)NC * B;
+    if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
+    ts_control_kernel<<<(unsigned)grid, TS_CTL_THREADS, 0, st>>>(d_params, B, sr, (long long)N, K, NC, table, hdr,
+                                                                static_cast<ts_agg *>(agg), epoch, params_human,
+                                                                dbg_ctl, d_active, full);
     return cudaGetLastError();
 }
