@@ -36,17 +36,38 @@ __device__ __forceinline__ void ts_bulk_store(void *gdst, const void *ssrc, uint
     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
-// sin(th) for th in [-pi/2, pi/2], odd polynomial: relative accuracy ~1e-7 down to th -> 0, which
-// the square/saw needs (its tanh has slope up to ~1e5 per cycle at the zero crossings, H4).
-__device__ __forceinline__ float ts_sin_poly(float th) {
-    const float t2 = th * th;
-    float p = -2.5052108e-8f;                // -1/11!
-    p = fmaf(p, t2, 2.7557319e-6f);          //  1/9!
-    p = fmaf(p, t2, -1.9841270e-4f);         // -1/7!
-    p = fmaf(p, t2, 8.3333333e-3f);          //  1/5!
-    p = fmaf(p, t2, -1.6666667e-1f);         // -1/3!
-    return fmaf(th * t2, p, th);
+// ---- packed fp32x2 arithmetic (Blackwell FFMA2 / FMUL2 / FADD2): one issue slot for two samples -----
+typedef unsigned long long ts_f2;
+__device__ __forceinline__ ts_f2 ts_pack(float lo, float hi) {
+    ts_f2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
 }
+__device__ __forceinline__ void ts_unpack(ts_f2 v, float &lo, float &hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ ts_f2 ts_fma2(ts_f2 a, ts_f2 b, ts_f2 c) {
+    ts_f2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ ts_f2 ts_mul2(ts_f2 a, ts_f2 b) {
+    ts_f2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ ts_f2 ts_add2(ts_f2 a, ts_f2 b) {
+    ts_f2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ ts_f2 ts_dup(float c) { return ts_pack(c, c); }
+
+// sin(th) for th in [-pi/2, pi/2] as th + th^3 q(th^2), q minimax of degree 3 (fit of (sin x / x - 1) / x^2 with
+// relative weighting): relative accuracy 1.2e-7 in fp32 down to th -> 0, which the square/saw needs (its tanh
+// has slope up to ~1e5 per cycle at the zero crossings, H4).
+constexpr float SIN_C3 = -0.16666659712791443f, SIN_C5 = 0.008333087898790836f, SIN_C7 = -0.00019811101083178073f,
+                SIN_C9 = 2.6089039693033556e-06f;
 
 template <int MODE>
 __global__ void __launch_bounds__(TS_AUDIO_THREADS)
@@ -91,6 +112,7 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
         {   // hop to the q-th run of the interval: 20 samples per hop in closed form
             const double g1 = v1.y, g2 = v3.y;
             const double e20a = e1a * g1, e20b = e1b * g2;
+#pragma unroll 1
             for (int i = 0; i < q; ++i) {
                 p1 = fma(w1, g1, p1);
                 w1 = fma(w1, e20a, w1);
@@ -103,44 +125,73 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
         const float da1 = (A1.x - A0.x) * (1.0f / TS_R), da2 = (A1.y - A0.y) * (1.0f / TS_R),
                     da3 = (A1.z - A0.z) * (1.0f / TS_R);
         float a1 = fmaf(A1.x - A0.x, mf, A0.x), a2 = fmaf(A1.y - A0.y, mf, A0.y), a3 = fmaf(A1.z - A0.z, mf, A0.z);
-        const float shape = hd.shape, tanh_c = hd.tanh_c;
         const uint32_t blk0 = (uint32_t)(n0 >> 2);
+        // Biased accumulators: P = MAGIC + phi keeps frac(phi) in the low mantissa word at every step (the add
+        // rounds to 2^-32 / 2^-33 of a cycle: <= 20 * 2^-33 = 2.3e-9 cycles over a run, budget 1e-8, H4).
+        double P1 = p1 + MAGIC32, P2 = p2 + MAGIC33;
 
+        if (MODE == 0) {
+            const ts_f2 SHAPE = ts_dup(hd.shape), TANH_C = ts_dup(hd.tanh_c), ONE = ts_dup(1.0f);
+            const uint32_t one_bits = 0x3f800000u;
+            ts_f2 G1 = ts_pack(a1, a1 + da1), G2 = ts_pack(a2, a2 + da2), G3 = ts_pack(a3, a3 + da3);
+            const ts_f2 DG1 = ts_dup(2.0f * da1), DG2 = ts_dup(2.0f * da2), DG3 = ts_dup(2.0f * da3);
+            ulonglong2 *my2 = reinterpret_cast<ulonglong2 *>(my);
 #pragma unroll
-        for (int g = 0; g < TS_RUN / 4; ++g) {
-            uint32_t nz[4];
-            if (MODE == 0) ts_philox4x32_10(blk0 + g, 0u, 0u, 1u, hd.nk0, hd.nk1, nz);  // S12
-            float o[4];
+            for (int g = 0; g < TS_RUN / 4; ++g) {
+                uint32_t nz[4];
+                ts_philox4x32_10(blk0 + g, 0u, 0u, 1u, hd.nk0, hd.nk1, nz);  // S12
+                ts_f2 O[2];
 #pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                if (MODE == 0) {
-                    // ---- S10 sine VCO: frac(phi) as signed Q0.32 straight from the fp64 mantissa
-                    const int x1 = __double2loint(p1 + MAGIC32);
-                    const float y1 = __sinf((float)x1 * 1.4629180792671596e-9f);  // 2 pi 2^-32
-                    // ---- S11 square/saw VCO: reduce to the nearest half cycle (H4)
-                    const double t = p2 + MAGIC33;
-                    const int lo = __double2loint(t), hi = __double2hiint(t);
-                    const uint32_t sgn = (((uint32_t)hi << 31) ^ (uint32_t)lo) & 0x80000000u;
-                    const float th = (float)lo * 7.314590396335798e-10f;  // 2 pi 2^-33, th in [-pi/2, pi/2)
-                    const float sn = __uint_as_float(__float_as_uint(ts_sin_poly(th)) ^ sgn);
-                    const float cs = __uint_as_float(__float_as_uint(__cosf(th)) ^ sgn);
-                    const float ex = ts_ex2(tanh_c * sn);
-                    const float th2 = fmaf(-2.0f, ts_rcp(1.0f + ex), 1.0f);  // tanh((pi/2) k sin)
-                    const float y2 = th2 * fmaf(shape, cs, 1.0f);
-                    // ---- S12 noise value, S13 VCAs, S14 mixer (gains already carry the mixer levels)
-                    const float z = fmaf((float)(nz[s] >> 8), 1.0f / 8388608.0f, -1.0f);
-                    o[s] = fmaf(a3, z, fmaf(a2, y2, a1 * y1));
-                    a1 += da1; a2 += da2; a3 += da3;
-                } else {
-                    const long long n = n0 + g * 4 + s;
-                    const double ph = (MODE == 1) ? p1 : p2;
-                    if (n < N) dbg_phase[(size_t)voice * N + n] = ph - floor(ph);
+                for (int h = 0; h < 2; ++h) {
+                    // ---- S9: phase accumulation for two consecutive samples (fp64, geometric increments)
+                    const int xa = __double2loint(P1);
+                    const int la = __double2loint(P2), ha = __double2hiint(P2);
+                    P1 += w1; w1 = fma(w1, e1a, w1);
+                    P2 += w2; w2 = fma(w2, e1b, w2);
+                    const int xb = __double2loint(P1);
+                    const int lb = __double2loint(P2), hb = __double2hiint(P2);
+                    P1 += w1; w1 = fma(w1, e1a, w1);
+                    P2 += w2; w2 = fma(w2, e1b, w2);
+                    // ---- S10 sine VCO: frac(phi) is the signed Q0.32 in the low word
+                    float r1a, r1b;
+                    ts_unpack(ts_mul2(ts_pack((float)xa, (float)xb), ts_dup(1.4629180792671596e-9f)), r1a, r1b);  // 2 pi 2^-32
+                    const ts_f2 Y1 = ts_pack(__sinf(r1a), __sinf(r1b));
+                    // ---- S11 square/saw VCO: low word = signed Q0.32 of the nearest HALF cycle (H4); the parity of
+                    // that half cycle (bit 0 of the high word, +1 if the low word is negative) is the sign sigma.
+                    const uint32_t sa = (((uint32_t)la + ((uint32_t)ha << 31)) & 0x80000000u) | one_bits;
+                    const uint32_t sb = (((uint32_t)lb + ((uint32_t)hb << 31)) & 0x80000000u) | one_bits;
+                    const ts_f2 SIG = ts_pack(__uint_as_float(sa), __uint_as_float(sb));
+                    const ts_f2 TH = ts_mul2(ts_pack((float)la, (float)lb), ts_dup(7.314590396335798e-10f));  // 2 pi 2^-33
+                    const ts_f2 T2 = ts_mul2(TH, TH);
+                    ts_f2 Q = ts_fma2(T2, ts_dup(SIN_C9), ts_dup(SIN_C7));
+                    Q = ts_fma2(Q, T2, ts_dup(SIN_C5));
+                    Q = ts_fma2(Q, T2, ts_dup(SIN_C3));
+                    const ts_f2 SN = ts_fma2(ts_mul2(TH, T2), Q, TH);  // sin(th), th in [-pi/2, pi/2)
+                    float tha, thb, ea, eb, da, db;
+                    ts_unpack(TH, tha, thb);
+                    const ts_f2 CS = ts_pack(__cosf(tha), __cosf(thb));
+                    ts_unpack(ts_mul2(SN, TANH_C), ea, eb);
+                    ts_unpack(ts_add2(ts_pack(ts_ex2(ea), ts_ex2(eb)), ONE), da, db);
+                    // tanh((pi/2) k sin) = 1 - 2 / (1 + 2^(c sin));  y2 = sigma tanh (1 + s sigma cos) = tanh (sigma + s cos)
+                    const ts_f2 TNH = ts_fma2(ts_pack(ts_rcp(da), ts_rcp(db)), ts_dup(-2.0f), ONE);
+                    const ts_f2 Y2 = ts_mul2(TNH, ts_fma2(SHAPE, CS, SIG));
+                    // ---- S12 noise value (RZ conversion keeps the top 24 bits of x when x >= 2^31 and a few more
+                    // below: within 2^-24 of (x >> 8) 2^-23 - 1), S13 VCAs, S14 mixer (gains carry the mixer levels)
+                    const ts_f2 Z = ts_fma2(ts_pack(__uint2float_rz(nz[2 * h]), __uint2float_rz(nz[2 * h + 1])),
+                                            ts_dup(4.656612873077393e-10f), ts_dup(-1.0f));
+                    O[h] = ts_fma2(G3, Z, ts_fma2(G2, Y2, ts_mul2(G1, Y1)));
+                    G1 = ts_add2(G1, DG1); G2 = ts_add2(G2, DG2); G3 = ts_add2(G3, DG3);
                 }
-                // ---- S9: phase accumulation; increments are geometric inside the interval
-                p1 += w1; w1 = fma(w1, e1a, w1);
-                p2 += w2; w2 = fma(w2, e1b, w2);
+                my2[g] = make_ulonglong2(O[0], O[1]);
             }
-            if (MODE == 0) my[g] = make_float4(o[0], o[1], o[2], o[3]);
+        } else {
+            for (int i = 0; i < TS_RUN; ++i) {
+                const long long n = n0 + i;
+                const double ph = (MODE == 1) ? (P1 - MAGIC32) : (P2 - MAGIC33);
+                if (n < N) dbg_phase[(size_t)voice * N + n] = ph - floor(ph);
+                P1 += w1; w1 = fma(w1, e1a, w1);
+                P2 += w2; w2 = fma(w2, e1b, w2);
+            }
         }
     } else if (MODE == 0) {
 #pragma unroll

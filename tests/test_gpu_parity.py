@@ -120,7 +120,8 @@ def test_phase_c1(T):
             r = O.render_voice(u[b], nk[b], wl.sr, wl.N, neb, want_phase=True)
             d = np.abs(ph[b] - r[f"phase{vco}"])
             d = np.minimum(d, 1 - d)
-            assert d.max() < 1e-9, (vco, b, d.max())
+            # the audio kernel accumulates phase on a 2^-32 (VCO 1) / 2^-33 (VCO 2) cycle grid: <= 20 * 2^-33 per run
+            assert d.max() < 3e-9, (vco, b, d.max())
 
 
 # ---------------------------------------------------------------------------------- audio parity, all configs
