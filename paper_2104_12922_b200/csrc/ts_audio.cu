@@ -68,11 +68,16 @@ __device__ __forceinline__ ts_f2 ts_dup(float c) { return ts_pack(c, c); }
 // has slope up to ~1e5 per cycle at the zero crossings, H4).
 constexpr float SIN_C3 = -0.16666659712791443f, SIN_C5 = 0.008333087898790836f, SIN_C7 = -0.00019811101083178073f,
                 SIN_C9 = 2.6089039693033556e-06f;
+// cos(th) on the same interval as 1 + th^2 r(th^2), r minimax of degree 3: absolute accuracy 1.7e-7 in fp32.  A
+// polynomial instead of MUFU.COS: same issue slots (4 FFMA2 per sample pair), but the XU pipe, which the
+// remaining sin / ex2 / rcp keep busy half the time, gets 25 % less work.
+constexpr float COS_C2 = -0.4999993145465851f, COS_C4 = 0.041663989424705505f, COS_C6 = -0.001385591458529234f,
+                COS_C8 = 2.319407394679729e-05f;
 
 template <int MODE>
 __global__ void __launch_bounds__(TS_AUDIO_THREADS)
 ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ hdr, int B, long long N, int K,
-                float *__restrict__ audio, double *__restrict__ dbg_phase, int aligned) {
+                float *__restrict__ audio, double *__restrict__ dbg_phase, int aligned, uint32_t one_bits) {
     __shared__ __align__(128) float4 stage[TS_TILE / 4];
 
     const int voice = blockIdx.x % B;  // time-major grid: the audible (expensive) tiles are dispatched first
@@ -132,7 +137,6 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
 
         if (MODE == 0) {
             const ts_f2 SHAPE = ts_dup(hd.shape), TANH_C = ts_dup(hd.tanh_c), ONE = ts_dup(1.0f);
-            const uint32_t one_bits = 0x3f800000u;
             ts_f2 G1 = ts_pack(a1, a1 + da1), G2 = ts_pack(a2, a2 + da2), G3 = ts_pack(a3, a3 + da3);
             const ts_f2 DG1 = ts_dup(2.0f * da1), DG2 = ts_dup(2.0f * da2), DG3 = ts_dup(2.0f * da3);
             ulonglong2 *my2 = reinterpret_cast<ulonglong2 *>(my);
@@ -167,9 +171,11 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
                     Q = ts_fma2(Q, T2, ts_dup(SIN_C5));
                     Q = ts_fma2(Q, T2, ts_dup(SIN_C3));
                     const ts_f2 SN = ts_fma2(ts_mul2(TH, T2), Q, TH);  // sin(th), th in [-pi/2, pi/2)
-                    float tha, thb, ea, eb, da, db;
-                    ts_unpack(TH, tha, thb);
-                    const ts_f2 CS = ts_pack(__cosf(tha), __cosf(thb));
+                    float ea, eb, da, db;
+                    ts_f2 CS = ts_fma2(T2, ts_dup(COS_C8), ts_dup(COS_C6));
+                    CS = ts_fma2(CS, T2, ts_dup(COS_C4));
+                    CS = ts_fma2(CS, T2, ts_dup(COS_C2));
+                    CS = ts_fma2(CS, T2, ONE);
                     ts_unpack(ts_mul2(SN, TANH_C), ea, eb);
                     ts_unpack(ts_add2(ts_pack(ts_ex2(ea), ts_ex2(eb)), ONE), da, db);
                     // tanh((pi/2) k sin) = 1 - 2 / (1 + 2^(c sin));  y2 = sigma tanh (1 + s sigma cos) = tanh (sigma + s cos)
@@ -219,10 +225,10 @@ cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int
     if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = (N % 4 == 0) && ((reinterpret_cast<uintptr_t>(audio) & 15u) == 0);
     if (mode == 0)
-        ts_audio_kernel<0><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned);
+        ts_audio_kernel<0><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u);
     else if (mode == 1)
-        ts_audio_kernel<1><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, 0);
+        ts_audio_kernel<1><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, 0, 0x3f800000u);
     else
-        ts_audio_kernel<2><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, 0);
+        ts_audio_kernel<2><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, 0, 0x3f800000u);
     return cudaGetLastError();
 }
