@@ -76,6 +76,7 @@ struct ts_voice_consts {
     double dq_f[2], dq_d[2];  // LFO frequency / cr and rate-mod depth / cr (cycles per tick)
     double g[3];              // VCA gains: mixer level / level sum; VCO2 also carries (1 - s/2) of S11
     int jsil;                 // first tick at which the voice is silent for good (== K if never)
+    int slow;                 // some ADSR alpha <= 0: use the generic power
 };
 
 // S4 ramp(t,s,d)^alpha.  pow(0,a) = 0 and pow(1,a) = 1 exactly for a > 0, so the saturated ends skip pow.
@@ -100,6 +101,33 @@ __device__ __forceinline__ double ts_adsr(double t, int e, const ts_voice_consts
     if (a == 0.0) return 0.0;
     const double d = ts_ramp_pow(t, rs[2], rd[2], ri[2], al, T);
     return a * (1.0 - (1.0 - S) * d) * (1.0 - r);
+}
+
+// x^a for x in [0,1], a > 0, without branches: exact 0 and 1 at the ends (S4 needs both: E = 0 exactly once the
+// release is over), clamped log2/exp2 in between.  Twelve of these per tick are independent chains, so the
+// fp64 latency that dominates this kernel overlaps instead of adding up.
+__device__ __forceinline__ double ts_pow01_sel(double x, double a, const ts_math_tables *T) {
+    const double xc = fmin(fmax(x, 1e-300), 1.0);
+    double p = ts_exp2(fmax(a * ts_log2(xc, T), -1000.0), T);
+    p = (x >= 1.0) ? 1.0 : p;
+    return (x <= 0.0) ? 0.0 : p;
+}
+__device__ __forceinline__ double ts_ramp_lin(double t, double s, double d, double invd) {  // S4 ramp(t,s,d)
+    const double x = t - s;
+    return (x >= d) ? 1.0 : ((x <= 0.0) ? 0.0 : x * invd);
+}
+// Same E(t) as ts_adsr for alpha > 0.  While the attack ramp is below 1 the decay ramp is 0 and afterwards the
+// attack ramp is 1, so ONE power serves both: two powers per envelope instead of three.
+__device__ __forceinline__ double ts_adsr_fast(double t, int e, const ts_voice_consts &V, const ts_math_tables *T) {
+    const double S = V.h[4 + 5 * e], al = V.h[6 + 5 * e];
+    const double *rs = &V.rs[3 * e], *rd = &V.rd[3 * e], *ri = &V.rinv[3 * e];
+    const double r = ts_ramp_lin(t, rs[0], rd[0], ri[0]);
+    const double a = ts_ramp_lin(t, rs[1], rd[1], ri[1]);
+    const double d = ts_ramp_lin(t, rs[2], rd[2], ri[2]);
+    const bool in_attack = a < 1.0;
+    const double pm = ts_pow01_sel(in_attack ? a : d, al, T), pr = ts_pow01_sel(r, al, T);
+    const double pa = in_attack ? pm : 1.0, pd = in_attack ? 0.0 : pm;
+    return pa * (1.0 - (1.0 - S) * pd) * (1.0 - pr);
 }
 
 // frac of a double as Q0.64
@@ -159,9 +187,28 @@ __device__ __forceinline__ void ts_lookback(const ts_agg *slots, int c, unsigned
 }
 
 // S6 LFO value at phase p in [0,1): blend of the five shapes with pre-normalised weights (D11).
+// sin(2 pi p) for p in [0,1) without branches: y = 2p - 1, sin(2 pi p) = -sin(pi y); |y| > 1/2 is folded back with
+// sin(pi - x) = sin x, then the Taylor series of sin(pi y) to y^19 (truncation 2.6e-16 at |y| = 1/2).
+__device__ __forceinline__ double ts_sin2pi(double p) {
+    double y = 2.0 * p - 1.0;
+    y = (fabs(y) > 0.5) ? copysign(1.0, y) - y : y;
+    const double y2 = y * y;
+    double q = -2.29484289972698730e-08;
+    q = fma(q, y2, 7.95205400147551261e-07);
+    q = fma(q, y2, -2.19153534478302173e-05);
+    q = fma(q, y2, 4.66302805767612554e-04);
+    q = fma(q, y2, -7.37043094571435044e-03);
+    q = fma(q, y2, 8.21458866111282326e-02);
+    q = fma(q, y2, -5.99264529320792105e-01);
+    q = fma(q, y2, 2.55016403987734552e+00);
+    q = fma(q, y2, -5.16771278004997026e+00);
+    q = fma(q, y2, 3.14159265358979312e+00);
+    return -(q * y);
+}
+
 __device__ __forceinline__ double ts_lfo_mix(double p, const double *wn) {
     const double t = p + 0.75;
-    double v = wn[0] * sinpi(2.0 * p);
+    double v = wn[0] * ts_sin2pi(p);
     v = fma(wn[1], 4.0 * fabs((t - floor(t)) - 0.5) - 1.0, v);
     v = fma(wn[2], 2.0 * p - 1.0, v);
     v = fma(wn[3], 1.0 - 2.0 * p, v);
@@ -243,6 +290,11 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
         while (j > 0 && (((double)((j - 1) * TS_R) / (double)sr) - D >= rl_max)) --j;
         if (full) j = K;  // debug exports: evaluate every tick
         V.jsil = (int)j;
+        {
+            int slow = 0;
+            for (int e = 0; e < 6; ++e) slow |= !(h[6 + 5 * e] > 0.0);
+            V.slow = slow;
+        }
         if (c == 0) {
             const long long n_act = (j * TS_R < N) ? j * TS_R : N;
             ts_vhdr hd;
@@ -271,10 +323,15 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
     unsigned long long dq1 = 0, dq2 = 0;
     if (live) {
         const double tau = (double)((long long)j * TS_R) / (double)sr;
+        if (V.slow) {  // some alpha <= 0 (custom nebula): generic path, uniform over the voice
 #pragma unroll 1
-        for (int e = 0; e < 6; ++e) Es[e][tid] = ts_adsr(tau, e, V, &MT);  // rolled: one copy of the pow code
+            for (int e = 0; e < 6; ++e) Es[e][tid] = ts_adsr(tau, e, V, &MT);
 #pragma unroll
-        for (int e = 0; e < 6; ++e) E[e] = Es[e][tid];
+            for (int e = 0; e < 6; ++e) E[e] = Es[e][tid];
+        } else {
+#pragma unroll
+            for (int e = 0; e < 6; ++e) E[e] = ts_adsr_fast(tau, e, V, &MT);
+        }
         const double d1 = fma(V.dq_d[0], E[3], V.dq_f[0]);
         const double d2 = fma(V.dq_d[1], E[5], V.dq_f[1]);
         dq1 = (unsigned long long)__double2ll_rn((d1 - rint(d1)) * 18446744073709551616.0);
@@ -286,10 +343,8 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
     __syncthreads();
     const unsigned long long q1 = ts_frac_q64(h[34]) + acc[0] + dq1, q2 = ts_frac_q64(h[42]) + acc[1] + dq2;
     if (live) {
-#pragma unroll 1
-        for (int l = 0; l < 2; ++l)  // rolled: one copy of the sinpi code
-            Es[l][tid] = Es[2 + 2 * l][tid] * ts_lfo_mix(ts_q64_to_double(l ? q2 : q1), V.lfo_w[l]);
-        const double L1 = Es[0][tid], L2 = Es[1][tid];
+        const double L1 = E[2] * ts_lfo_mix(ts_q64_to_double(q1), V.lfo_w[0]);
+        const double L2 = E[4] * ts_lfo_mix(ts_q64_to_double(q2), V.lfo_w[1]);
         double M[5];
 #pragma unroll
         for (int d = 0; d < 5; ++d)
