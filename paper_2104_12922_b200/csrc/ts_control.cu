@@ -19,11 +19,20 @@
 #include "ts_common.cuh"
 #include "ts_math.cuh"
 
-__constant__ ts_range c_nebula[TS_NPARAM];
-__constant__ ts_math_tables c_math;
+// Both tables live in GLOBAL memory: every thread reads its own entry, which the constant cache would serialise
+// (one distinct address per cycle; it showed up as 34 % ADU-pipe load), while LDG coalesces it.
+struct ts_range_dev {
+    double lo, hi, curve, inv_curve;  // inv_curve = 1 / curve, divided once on the host (IEEE: same bits as here)
+    long long symmetric;
+};
+__device__ ts_range_dev c_nebula[TS_NPARAM];
+__device__ ts_math_tables c_math;
 
 cudaError_t ts_upload_nebula(const ts_range *host78, cudaStream_t st) {
-    return cudaMemcpyToSymbolAsync(c_nebula, host78, sizeof(ts_range) * TS_NPARAM, 0, cudaMemcpyHostToDevice, st);
+    static ts_range_dev D[TS_NPARAM];  // static: the async copy reads it after this function returns
+    for (int i = 0; i < TS_NPARAM; ++i)
+        D[i] = ts_range_dev{host78[i].lo, host78[i].hi, host78[i].curve, 1.0 / host78[i].curve, (long long)host78[i].symmetric};
+    return cudaMemcpyToSymbolAsync(c_nebula, D, sizeof D, 0, cudaMemcpyHostToDevice, st);
 }
 
 cudaError_t ts_upload_math_tables(cudaStream_t st) {
@@ -52,16 +61,16 @@ __device__ __forceinline__ double ts_pow_unit(double x, double a, const ts_math_
     return ts_pow01(x, a, T);
 }
 
-__device__ double ts_map(double u, const ts_range &r, const ts_math_tables *T) {
+__device__ __forceinline__ double ts_map(double u, const ts_range_dev &r, const ts_math_tables *T) {
     if (!(u >= 0.0)) u = 0.0;
     if (u > 1.0) u = 1.0;
     if (!r.symmetric) {
-        const double v = (r.curve == 1.0) ? u : ts_pow_unit(u, 1.0 / r.curve, T);
+        const double v = (r.curve == 1.0) ? u : ts_pow_unit(u, r.inv_curve, T);
         return __dadd_rn(r.lo, __dmul_rn(r.hi - r.lo, v));
     }
     const double d = __dadd_rn(__dmul_rn(2.0, u), -1.0);
     const double a = fabs(d);
-    const double v = (r.curve == 1.0) ? a : ts_pow_unit(a, 1.0 / r.curve, T);
+    const double v = (r.curve == 1.0) ? a : ts_pow_unit(a, r.inv_curve, T);
     const double s = (d > 0.0) ? 1.0 : ((d < 0.0) ? -1.0 : 0.0);
     return __dadd_rn((r.lo + r.hi) / 2.0, __dmul_rn((r.hi - r.lo) / 2.0, s * v));
 }
@@ -273,21 +282,31 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
         const double *w = &h[48 + 4 * d];
         const double den = ((w[0] + w[1]) + w[2]) + w[3];
         V.mix_w[d][sidx] = (den == 0.0) ? 0.0 : w[sidx] / den;
-    } else if (tid >= 97 && tid < 100) {
-        const int i = tid - 97;
+    } else if (tid >= 46 && tid < 49) {
+        const int i = tid - 46;
         const double lsum = (h[75] + h[76]) + h[77];
         const double gi = (lsum == 0.0) ? 0.0 : h[75 + i] / lsum;
         V.g[i] = (i == 1) ? gi * (1.0 - h[74] / 2.0) : gi;  // VCO2 carries (1 - s/2) of S11
-    } else if (tid == 96) {
+    } else if (tid >= 96) {
         // The voice is silent for good once the release of all four audible envelopes is over (their
-        // ramp is 1, so E = 0 exactly): adsr1, adsr2, lfo1_amp, lfo2_amp.
+        // ramp is 1, so E = 0 exactly): adsr1, adsr2, lfo1_amp, lfo2_amp.  jsil = first tick with
+        // (tau - D) >= rl_max, evaluated exactly as S4's ramp does; the predicate is monotone in j, so the 32 lanes
+        // of this warp test 32 candidates around the estimate at once (one fp64 division each, not a serial walk).
         const double rl_max = fmax(fmax(h[2 + 3], h[7 + 3]), fmax(h[12 + 3], h[22 + 3]));
-        long long j = (long long)floor((D + rl_max) * cr) - 2;
-        if (j < 0) j = 0;
-        if (j > K - 1) j = K - 1;
-        // first tick with (tau - D) >= rl_max, evaluated exactly as S4's ramp does
-        while (j < K && !(((double)(j * TS_R) / (double)sr) - D >= rl_max)) ++j;
-        while (j > 0 && (((double)((j - 1) * TS_R) / (double)sr) - D >= rl_max)) --j;
+        const int lane = tid - 96;
+        long long je = (long long)floor((D + rl_max) * cr) - 8;
+        if (je > K) je = K;
+        if (je < 0) je = 0;
+        auto silent_at = [&](long long jj) { return jj >= K || (((double)(jj * TS_R) / (double)sr) - D >= rl_max); };
+        const unsigned int hit = __ballot_sync(0xffffffffu, silent_at(je + lane));
+        long long j = hit ? je + (__ffs(hit) - 1) : je + 32;
+        if (lane == 0 && (hit & 1u)) {  // estimate off (cannot happen for finite parameters): walk
+            while (j > 0 && silent_at(j - 1)) --j;
+        } else if (lane == 0 && !hit) {
+            while (!silent_at(j)) ++j;
+        }
+        j = __shfl_sync(0xffffffffu, j, 0);
+        if (tid == 96) {  // one thread writes the results
         if (full) j = K;  // debug exports: evaluate every tick
         V.jsil = (int)j;
         {
@@ -309,6 +328,7 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
             hd.pad[0] = hd.pad[1] = 0;
             hdr[v] = hd;
             if (d_active) atomicAdd(d_active, (unsigned long long)n_act);
+        }
         }
     }
     __syncthreads();
