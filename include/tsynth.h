@@ -76,6 +76,16 @@ int ts_render(const ts_voice *d_params, int B, int sr, double seconds, ts_out ou
 int ts_render_host(uint64_t seed, uint64_t batch_index, int B, int sr, double seconds,
                    float *host_audio, ts_voice *host_params);
 
+/* Streaming corpus generation ("generated on the fly from a batch index"; BASELINE.json configs[2]):
+ * batches first_batch .. first_batch + n_batches - 1 of B voices each, batch i sampled and rendered into ring slot
+ * i % n_ring: records at d_params_ring[(i % n_ring) * B], audio at d_audio_ring[(i % n_ring) * B * N].  Same
+ * results as n_batches calls of ts_sample_params + ts_render, but consecutive batches run on two internal streams
+ * with a workspace each, so the control stage of one batch overlaps the audio stage of the previous one.  The
+ * work is ordered after everything queued on the set stream and the set stream continues after it; the call
+ * itself does not synchronise.  A slot is overwritten n_ring batches later: consume it before that. */
+int ts_corpus_render(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds,
+                     ts_voice *d_params_ring, float *d_audio_ring, int n_ring);
+
 /* D17: N = llround(sr*seconds);  S5: K = ceil(N/TS_R) + 1 control ticks. */
 int64_t ts_num_samples(int sr, double seconds);
 int64_t ts_num_ticks(int64_t N);
@@ -94,7 +104,8 @@ void ts_shutdown(void);                            /* frees the workspace       
 int ts_set_timing(int enable);
 int ts_last_kernel_ms(float host_ms[2]);
 /* Counters of the LAST ts_render (host): [0] kernels launched, [1] voice chunks,
- * [2] audio samples in the active (non-silent) prefix summed over voices (valid after ts_sync). */
+ * [2] audio samples in the active (non-silent) prefix summed over voices (counted only while timing is
+ * enabled with ts_set_timing; valid after ts_sync). */
 int ts_last_stats(int64_t host_stats[3]);
 
 /* Debug exports used only by the parity tests. */

@@ -28,7 +28,7 @@ class _Out(C.Structure):
     _fields_ = [("audio", C.c_void_p), ("params_human", C.c_void_p)]
 
 
-EXPORTS = ["ts_sample_params", "ts_render", "ts_render_host", "ts_num_samples", "ts_num_ticks", "ts_set_stream",
+EXPORTS = ["ts_sample_params", "ts_render", "ts_render_host", "ts_corpus_render", "ts_num_samples", "ts_num_ticks", "ts_set_stream",
            "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes", "ts_last_error", "ts_sync", "ts_shutdown",
            "ts_set_timing", "ts_last_kernel_ms", "ts_last_stats", "ts_debug_noise_u32", "ts_debug_controls",
            "ts_debug_phase"]
@@ -51,6 +51,7 @@ def lib():
     L.ts_sample_params.argtypes = [u64, u64, i32, vp]
     L.ts_render.argtypes = [vp, i32, i32, f64, _Out]
     L.ts_render_host.argtypes = [u64, u64, i32, i32, f64, vp, vp]
+    L.ts_corpus_render.argtypes = [u64, u64, i32, i32, i32, f64, vp, vp, i32]
     L.ts_num_samples.argtypes = [i32, f64]
     L.ts_num_samples.restype = C.c_int64
     L.ts_num_ticks.argtypes = [C.c_int64]
@@ -196,6 +197,23 @@ def ts_render_host(seed: int, batch_index: int, B: int, sr: int, seconds: float,
     _use_current_stream(torch.device("cuda", torch.cuda.current_device()))
     _check(lib().ts_render_host(seed, batch_index, B, sr, float(seconds), C.c_void_p(ap), C.c_void_p(pp) if pp else None))
     return host_audio
+
+
+def ts_corpus_render(seed: int, first_batch: int, n_batches: int, sr: int, seconds: float, params_ring, audio_ring):
+    """Streams n_batches consecutive batches into the rings: params_ring [R, B, 80], audio_ring [R, B, N] (CUDA fp32)."""
+    torch = _torch()
+    if not (params_ring.is_cuda and params_ring.dtype == torch.float32 and params_ring.dim() == 3
+            and params_ring.shape[2] == REC_FLOATS and params_ring.is_contiguous()):
+        raise TsynthError("params_ring must be a contiguous CUDA float32 tensor [R, B, 80]")
+    R_, B = int(params_ring.shape[0]), int(params_ring.shape[1])
+    N = ts_num_samples(sr, seconds)
+    if not (audio_ring.is_cuda and audio_ring.dtype == torch.float32 and audio_ring.is_contiguous()
+            and tuple(audio_ring.shape) == (R_, B, N)):
+        raise TsynthError("audio_ring must be a contiguous CUDA float32 tensor [R, B, N]")
+    _use_current_stream(params_ring.device)
+    _check(lib().ts_corpus_render(seed, first_batch, n_batches, B, sr, float(seconds), C.c_void_p(params_ring.data_ptr()),
+                                  C.c_void_p(audio_ring.data_ptr()), R_))
+    return audio_ring
 
 
 def ts_debug_noise_u32(key, n0: int, count: int, device="cuda:0"):

@@ -8,17 +8,35 @@
 
 namespace {
 
-struct ts_state {
+// A lane = a workspace with the stream(s) that use it, so that two batches can be in flight at once.
+// Lane 0 serves ts_render / ts_render_host on the caller's stream.  Lanes 1 and 2 serve ts_corpus_render: they
+// share one HIGH-priority stream for the sampler and the (latency-bound) control kernel and one LOW-priority
+// stream for the (issue-bound) audio kernel, so that the control stage of batch i+1 is dispatched into the SMs
+// while the audio stage of batch i still runs and fills the issue slots it leaves idle.
+struct ts_lane {
     cudaStream_t stream = nullptr;
+    void *ws = nullptr;
+    size_t ws_bytes = 0;
+    unsigned int epoch = 0;  // look-back flag value of the latest control launch on this workspace
+    unsigned long long *d_active = nullptr;
+    unsigned long long *h_active = nullptr;  // pinned
+    // lanes 1, 2 (ts_corpus_render): the audio kernel goes to its own low-priority stream
+    cudaStream_t audio_stream = nullptr;
+    cudaEvent_t ctl_done = nullptr, aud_done = nullptr;
+    bool aud_pending = false;  // aud_done was recorded after the latest audio kernel that reads this workspace
+};
+constexpr int TS_LANES = 3;
+
+struct ts_state {
     char err[512] = "";
     ts_range nebula[TS_NPARAM];
     bool nebula_init = false;
-    bool nebula_dirty = true;  // device constant copy is stale
+    bool nebula_dirty = true;  // device copy is stale
     bool math_uploaded = false;
-    unsigned int epoch = 0;    // look-back flag value of the latest control launch
-    // workspace
-    void *ws = nullptr;
-    size_t ws_bytes = 0;
+    ts_lane lane[TS_LANES];
+    ts_lane *cur = &lane[0];
+    cudaEvent_t fork = nullptr;
+    cudaStream_t hi = nullptr, lo = nullptr;  // ts_corpus_render's internal streams
     // host staging for ts_render_host
     void *stage = nullptr;
     size_t stage_bytes = 0;
@@ -27,8 +45,6 @@ struct ts_state {
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
     float ms[2] = {0.f, 0.f};
     int64_t stats[3] = {0, 0, 0};
-    unsigned long long *d_active = nullptr;
-    unsigned long long *h_active = nullptr;  // pinned
 };
 ts_state S;
 
@@ -99,18 +115,18 @@ bool nebula_supported(int sr) {
 }
 
 int ensure_ws(size_t bytes) {
-    if (bytes <= S.ws_bytes) return TS_OK;
-    if (S.ws) cudaFree(S.ws);
-    S.ws = nullptr;
-    S.ws_bytes = 0;
-    if (cudaMalloc(&S.ws, bytes) != cudaSuccess) {
+    if (bytes <= S.cur->ws_bytes) return TS_OK;
+    if (S.cur->ws) cudaFree(S.cur->ws);
+    S.cur->ws = nullptr;
+    S.cur->ws_bytes = 0;
+    if (cudaMalloc(&S.cur->ws, bytes) != cudaSuccess) {
         cudaGetLastError();
         return fail(TS_ENOMEM, "workspace allocation failed%s");
     }
-    S.ws_bytes = bytes;
+    S.cur->ws_bytes = bytes;
     // look-back flags must never equal a future epoch: start from zeros and restart the epoch count
-    if (cudaMemsetAsync(S.ws, 0, bytes, S.stream) != cudaSuccess) return cuda_fail(cudaGetLastError(), "cudaMemsetAsync");
-    S.epoch = 0;
+    if (cudaMemsetAsync(S.cur->ws, 0, bytes, S.cur->stream) != cudaSuccess) return cuda_fail(cudaGetLastError(), "cudaMemsetAsync");
+    S.cur->epoch = 0;
     return TS_OK;
 }
 
@@ -144,17 +160,17 @@ int prepare_common(int sr) {
     ensure_nebula();
     if (!nebula_supported(sr)) return fail(TS_EINVAL, "nebula allows an oscillator increment above 2^18/R cycles per sample at this sr%s");
     if (S.nebula_dirty) {
-        TS_CUDA(ts_upload_nebula(S.nebula, S.stream));
+        TS_CUDA(ts_upload_nebula(S.nebula, S.cur->stream));
         S.nebula_dirty = false;
     }
     if (!S.math_uploaded) {
-        TS_CUDA(ts_upload_math_tables(S.stream));
+        TS_CUDA(ts_upload_math_tables(S.cur->stream));
         S.math_uploaded = true;
     }
-    if (!S.d_active) {
-        TS_CUDA(cudaMalloc(&S.d_active, sizeof(unsigned long long)));
-        TS_CUDA(cudaMallocHost(&S.h_active, sizeof(unsigned long long)));
-        *S.h_active = 0;
+    if (!S.cur->d_active) {
+        TS_CUDA(cudaMalloc(&S.cur->d_active, sizeof(unsigned long long)));
+        TS_CUDA(cudaMallocHost(&S.cur->h_active, sizeof(unsigned long long)));
+        *S.cur->h_active = 0;
     }
     return TS_OK;
 }
@@ -172,39 +188,54 @@ int render_impl(const ts_voice *d_params, int B, int sr, double seconds, float *
     size_t off_hdr, off_agg;
     rc = ensure_ws(ws_layout(Bc, K, &off_hdr, &off_agg));
     if (rc) return rc;
-    ts_tick *table = reinterpret_cast<ts_tick *>(S.ws);
-    ts_vhdr *hdr = reinterpret_cast<ts_vhdr *>(static_cast<char *>(S.ws) + off_hdr);
-    void *agg = static_cast<char *>(S.ws) + off_agg;
+    ts_tick *table = reinterpret_cast<ts_tick *>(S.cur->ws);
+    ts_vhdr *hdr = reinterpret_cast<ts_vhdr *>(static_cast<char *>(S.cur->ws) + off_hdr);
+    void *agg = static_cast<char *>(S.cur->ws) + off_agg;
 
     if (S.timing && mode == 0)
         for (auto &e : S.ev)
             if (!e) TS_CUDA(cudaEventCreate(&e));
     S.ms[0] = S.ms[1] = 0.f;
     int64_t launches = 0, chunks = 0;
-    TS_CUDA(cudaMemsetAsync(S.d_active, 0, sizeof(unsigned long long), S.stream));
-    if (mode == 3) TS_CUDA(cudaMemsetAsync(dbg, 0, (size_t)B * 5 * K * sizeof(double), S.stream));
+    const bool want_stats = S.timing;  // the active-sample count costs a memset and a copy per call
+    if (want_stats) TS_CUDA(cudaMemsetAsync(S.cur->d_active, 0, sizeof(unsigned long long), S.cur->stream));
+    if (mode == 3) TS_CUDA(cudaMemsetAsync(dbg, 0, (size_t)B * 5 * K * sizeof(double), S.cur->stream));
 
     for (int b0 = 0; b0 < B; b0 += Bc) {
         const int nb = (B - b0 < Bc) ? (B - b0) : Bc;
         const bool timed = S.timing && mode == 0;
-        if (timed) TS_CUDA(cudaEventRecord(S.ev[0], S.stream));
-        if (++S.epoch == 0) {  // wrapped after 2^32 launches: clear the flags and start over
-            TS_CUDA(cudaMemsetAsync(agg, 0, ts_control_agg_bytes(Bc, K), S.stream));
-            S.epoch = 1;
+        if (timed) TS_CUDA(cudaEventRecord(S.ev[0], S.cur->stream));
+        if (S.cur->aud_pending) {  // the audio kernel still reading this workspace's table goes first
+            TS_CUDA(cudaStreamWaitEvent(S.cur->stream, S.cur->aud_done, 0));
+            S.cur->aud_pending = false;
         }
-        TS_CUDA(ts_launch_control(d_params + b0, nb, sr, N, K, table, hdr, agg, S.epoch,
+        if (++S.cur->epoch == 0) {  // wrapped after 2^32 launches: clear the flags and start over
+            TS_CUDA(cudaMemsetAsync(agg, 0, ts_control_agg_bytes(Bc, K), S.cur->stream));
+            S.cur->epoch = 1;
+        }
+        TS_CUDA(ts_launch_control(d_params + b0, nb, sr, N, K, table, hdr, agg, S.cur->epoch,
                                   params_human ? params_human + (size_t)b0 * TS_NPARAM : nullptr,
-                                  mode == 3 ? dbg + (size_t)b0 * 5 * K : nullptr, S.d_active,
-                                  (mode == 1 || mode == 2) ? 1 : 0, S.stream));
+                                  mode == 3 ? dbg + (size_t)b0 * 5 * K : nullptr, want_stats ? S.cur->d_active : nullptr,
+                                  (mode == 1 || mode == 2) ? 1 : 0, S.cur->stream));
         ++launches;
-        if (timed) TS_CUDA(cudaEventRecord(S.ev[1], S.stream));
+        if (timed) TS_CUDA(cudaEventRecord(S.ev[1], S.cur->stream));
+        cudaStream_t ast = S.cur->stream;
+        if (S.cur->audio_stream && mode == 0) {  // hand over to the audio stream
+            ast = S.cur->audio_stream;
+            TS_CUDA(cudaEventRecord(S.cur->ctl_done, S.cur->stream));
+            TS_CUDA(cudaStreamWaitEvent(ast, S.cur->ctl_done, 0));
+        }
         if (mode != 3) {
             TS_CUDA(ts_launch_audio(table, hdr, nb, N, K, audio ? audio + (size_t)b0 * N : nullptr, mode,
-                                    (mode == 1 || mode == 2) ? dbg + (size_t)b0 * N : nullptr, S.stream));
+                                    (mode == 1 || mode == 2) ? dbg + (size_t)b0 * N : nullptr, ast));
             ++launches;
         }
+        if (ast != S.cur->stream) {  // the next control launch on this workspace will wait for this audio kernel
+            TS_CUDA(cudaEventRecord(S.cur->aud_done, ast));
+            S.cur->aud_pending = true;
+        }
         if (timed) {
-            TS_CUDA(cudaEventRecord(S.ev[2], S.stream));
+            TS_CUDA(cudaEventRecord(S.ev[2], S.cur->stream));
             TS_CUDA(cudaEventSynchronize(S.ev[2]));
             float a = 0.f, b = 0.f;
             TS_CUDA(cudaEventElapsedTime(&a, S.ev[0], S.ev[1]));
@@ -214,7 +245,9 @@ int render_impl(const ts_voice *d_params, int B, int sr, double seconds, float *
         }
         ++chunks;
     }
-    TS_CUDA(cudaMemcpyAsync(S.h_active, S.d_active, sizeof(unsigned long long), cudaMemcpyDeviceToHost, S.stream));
+    if (want_stats)
+        TS_CUDA(cudaMemcpyAsync(S.cur->h_active, S.cur->d_active, sizeof(unsigned long long), cudaMemcpyDeviceToHost,
+                                S.cur->stream));
     S.stats[0] = launches;
     S.stats[1] = chunks;
     return TS_OK;
@@ -230,7 +263,7 @@ int64_t ts_num_ticks(int64_t N) { return (N + TS_R - 1) / TS_R + 1; }
 int ts_sample_params(uint64_t seed, uint64_t batch_index, int B, ts_voice *d_params) {
     if (!d_params) return fail(TS_ENULL, "d_params is NULL%s");
     if (B <= 0) return fail(TS_EINVAL, "B must be positive%s");
-    TS_CUDA(ts_launch_sample(seed, batch_index * (uint64_t)B, B, d_params, S.stream));
+    TS_CUDA(ts_launch_sample(seed, batch_index * (uint64_t)B, B, d_params, S.cur->stream));
     return TS_OK;
 }
 
@@ -265,15 +298,69 @@ int ts_render_host(uint64_t seed, uint64_t batch_index, int B, int sr, double se
     if (rc) return rc;
     rc = render_impl(d_params, B, sr, seconds, d_audio, nullptr, 0, nullptr);
     if (rc) return rc;
-    TS_CUDA(cudaMemcpyAsync(host_audio, d_audio, abytes, cudaMemcpyDeviceToHost, S.stream));
+    TS_CUDA(cudaMemcpyAsync(host_audio, d_audio, abytes, cudaMemcpyDeviceToHost, S.cur->stream));
     if (host_params)
-        TS_CUDA(cudaMemcpyAsync(host_params, d_params, (size_t)B * sizeof(ts_voice), cudaMemcpyDeviceToHost, S.stream));
-    TS_CUDA(cudaStreamSynchronize(S.stream));
+        TS_CUDA(cudaMemcpyAsync(host_params, d_params, (size_t)B * sizeof(ts_voice), cudaMemcpyDeviceToHost, S.cur->stream));
+    TS_CUDA(cudaStreamSynchronize(S.cur->stream));
     return TS_OK;
 }
 
+int ts_corpus_render(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds,
+                     ts_voice *d_params_ring, float *d_audio_ring, int n_ring) {
+    if (!d_params_ring || !d_audio_ring) return fail(TS_ENULL, "NULL ring%s");
+    if (n_batches <= 0 || n_ring <= 0) return fail(TS_EINVAL, "n_batches and n_ring must be positive%s");
+    int64_t N;
+    int K;
+    int rc = check_sizes(B, sr, seconds, &N, &K);
+    if (rc) return rc;
+    S.cur = &S.lane[0];
+    rc = prepare_common(sr);  // nebula / tables go up on the caller's stream, before the fork
+    if (rc) return rc;
+    if (!S.fork) {
+        int lo_p = 0, hi_p = 0;
+        TS_CUDA(cudaDeviceGetStreamPriorityRange(&lo_p, &hi_p));  // numerically lower = higher priority
+        TS_CUDA(cudaStreamCreateWithPriority(&S.hi, cudaStreamNonBlocking, hi_p));
+        TS_CUDA(cudaStreamCreateWithPriority(&S.lo, cudaStreamNonBlocking, lo_p));
+        for (int l = 1; l < TS_LANES; ++l) {
+            S.lane[l].stream = S.hi;
+            S.lane[l].audio_stream = S.lo;
+            TS_CUDA(cudaEventCreateWithFlags(&S.lane[l].ctl_done, cudaEventDisableTiming));
+            TS_CUDA(cudaEventCreateWithFlags(&S.lane[l].aud_done, cudaEventDisableTiming));
+        }
+        TS_CUDA(cudaEventCreateWithFlags(&S.fork, cudaEventDisableTiming));
+    }
+    // fork: both internal streams start after everything already queued on the caller's stream
+    TS_CUDA(cudaEventRecord(S.fork, S.lane[0].stream));
+    TS_CUDA(cudaStreamWaitEvent(S.hi, S.fork, 0));
+    TS_CUDA(cudaStreamWaitEvent(S.lo, S.fork, 0));
+    const bool timing = S.timing;
+    S.timing = false;  // per-kernel events would serialise the streams
+    // Ring hazards: records are written by the sampler and read by the control kernel, both on `hi` in batch order;
+    // audio slots are written by the audio kernels, all on `lo` in batch order.  Nothing else to order.
+    for (int i = 0; i < n_batches && rc == TS_OK; ++i) {
+        ts_lane &L = S.lane[1 + (i & 1)];
+        const size_t slot = (size_t)(i % n_ring);
+        ts_voice *p = d_params_ring + slot * (size_t)B;
+        float *a = d_audio_ring + slot * (size_t)B * (size_t)N;
+        cudaError_t e = ts_launch_sample(seed, (first_batch + (uint64_t)i) * (uint64_t)B, B, p, L.stream);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "ts_launch_sample"); break; }
+        S.cur = &L;
+        rc = render_impl(p, B, sr, seconds, a, nullptr, 0, nullptr);
+    }
+    S.cur = &S.lane[0];
+    S.timing = timing;
+    // join: the caller's stream continues after both internal streams
+    TS_CUDA(cudaEventRecord(S.lane[1].ctl_done, S.hi));
+    TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.lane[1].ctl_done, 0));
+    TS_CUDA(cudaEventRecord(S.lane[2].ctl_done, S.lo));
+    TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.lane[2].ctl_done, 0));
+    S.stats[0] *= n_batches;  // kernels launched by this call (3 per batch and voice chunk: sampler counted below)
+    S.stats[0] += n_batches;
+    return rc;
+}
+
 int ts_set_stream(void *cuda_stream) {
-    S.stream = static_cast<cudaStream_t>(cuda_stream);
+    S.lane[0].stream = static_cast<cudaStream_t>(cuda_stream);
     return TS_OK;
 }
 
@@ -309,22 +396,34 @@ size_t ts_workspace_bytes(int B, int sr, double seconds) {
 const char *ts_last_error(void) { return S.err; }
 
 int ts_sync(void) {
-    TS_CUDA(cudaStreamSynchronize(S.stream));
-    if (S.h_active) S.stats[2] = (int64_t)*S.h_active;
+    TS_CUDA(cudaStreamSynchronize(S.lane[0].stream));
+    if (S.lane[0].h_active) S.stats[2] = (int64_t)*S.lane[0].h_active;
     return TS_OK;
 }
 
 void ts_shutdown(void) {
-    if (S.ws) cudaFree(S.ws);
+    for (int l = 0; l < TS_LANES; ++l) {
+        ts_lane &L = S.lane[l];
+        if (L.ws) cudaFree(L.ws);
+        if (L.d_active) cudaFree(L.d_active);
+        if (L.h_active) cudaFreeHost(L.h_active);
+        if (L.ctl_done) cudaEventDestroy(L.ctl_done);
+        if (L.aud_done) cudaEventDestroy(L.aud_done);
+        const cudaStream_t keep = (l == 0) ? L.stream : nullptr;
+        L = ts_lane();
+        L.stream = keep;
+    }
+    if (S.fork) { cudaEventDestroy(S.fork); S.fork = nullptr; }
+    if (S.hi) { cudaStreamDestroy(S.hi); S.hi = nullptr; }
+    if (S.lo) { cudaStreamDestroy(S.lo); S.lo = nullptr; }
     if (S.stage) cudaFree(S.stage);
-    if (S.d_active) cudaFree(S.d_active);
-    if (S.h_active) cudaFreeHost(S.h_active);
     for (auto &e : S.ev)
         if (e) { cudaEventDestroy(e); e = nullptr; }
-    S.ws = S.stage = nullptr;
-    S.ws_bytes = S.stage_bytes = 0;
-    S.d_active = S.h_active = nullptr;
+    S.stage = nullptr;
+    S.stage_bytes = 0;
+    S.cur = &S.lane[0];
     S.nebula_dirty = true;
+    S.math_uploaded = false;
 }
 
 int ts_set_timing(int enable) {
@@ -339,7 +438,7 @@ int ts_last_kernel_ms(float host_ms[2]) {
 }
 int ts_last_stats(int64_t host_stats[3]) {
     if (!host_stats) return fail(TS_ENULL, "host_stats is NULL%s");
-    if (S.h_active) S.stats[2] = (int64_t)*S.h_active;
+    if (S.lane[0].h_active) S.stats[2] = (int64_t)*S.lane[0].h_active;
     memcpy(host_stats, S.stats, sizeof S.stats);
     return TS_OK;
 }
@@ -347,7 +446,7 @@ int ts_last_stats(int64_t host_stats[3]) {
 int ts_debug_noise_u32(const uint32_t host_key[2], uint64_t n0, int count, uint32_t *d_out) {
     if (!host_key || !d_out) return fail(TS_ENULL, "NULL argument%s");
     if (count <= 0) return fail(TS_EINVAL, "count must be positive%s");
-    TS_CUDA(ts_launch_noise_debug(host_key[0], host_key[1], n0, count, d_out, S.stream));
+    TS_CUDA(ts_launch_noise_debug(host_key[0], host_key[1], n0, count, d_out, S.cur->stream));
     return TS_OK;
 }
 int ts_debug_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl) {

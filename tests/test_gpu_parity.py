@@ -281,3 +281,23 @@ def test_render_host_end_to_end(T):
     host = T.ts_render_host(4, 2, B, sr, seconds).numpy()
     u, nk = O.sample_params(4, 2, B)
     assert_parity(host, O.render_batch(u, nk, sr, N), "render_host")
+
+
+def test_corpus_render_matches_batch_by_batch(T):
+    """ts_corpus_render (two internal streams, ring of output slots) == ts_sample_params + ts_render, bitwise."""
+    import torch
+    T.ts_set_nebula(None)
+    B, sr, seconds, first = 5, 44100, 0.3, 7
+    N = O.num_samples(sr, seconds)
+    for n_ring, n_batches in ((2, 2), (3, 7), (4, 9)):
+        pr = torch.zeros((n_ring, B, 80), device="cuda")
+        ar = torch.full((n_ring, B, N), 9.0, device="cuda")
+        T.ts_corpus_render(3, first, n_batches, sr, seconds, pr, ar)
+        torch.cuda.synchronize()
+        for slot in range(n_ring):
+            i = max(k for k in range(n_batches) if k % n_ring == slot)      # the last batch written to this slot
+            p = T.ts_sample_params(3, first + i, B)
+            a = T.ts_render(p, sr, seconds)
+            assert torch.equal(pr[slot], p) and torch.equal(ar[slot], a), (n_ring, slot, i)
+    u, nk = O.sample_params(3, first + 8, B)                                 # and against the oracle
+    assert_parity(ar[0].cpu().numpy(), O.render_batch(u, nk, sr, N), "corpus")
