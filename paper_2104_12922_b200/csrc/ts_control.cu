@@ -134,7 +134,12 @@ __device__ __forceinline__ double ts_adsr_fast(double t, int e, const ts_voice_c
     const double a = ts_ramp_lin(t, rs[1], rd[1], ri[1]);
     const double d = ts_ramp_lin(t, rs[2], rd[2], ri[2]);
     const bool in_attack = a < 1.0;
-    const double pm = ts_pow01_sel(in_attack ? a : d, al, T), pr = ts_pow01_sel(r, al, T);
+    const double m = in_attack ? a : d;
+    // A power is evaluated only if some lane of the warp is strictly inside that ramp (32 consecutive ticks = 73 ms:
+    // during sustain, before the note-off and after the release nothing is).  Called by full warps only.
+    double pm = (m >= 1.0) ? 1.0 : 0.0, pr = (r >= 1.0) ? 1.0 : 0.0;
+    if (__any_sync(0xffffffffu, m > 0.0 && m < 1.0)) pm = ts_pow01_sel(m, al, T);
+    if (__any_sync(0xffffffffu, r > 0.0 && r < 1.0)) pr = ts_pow01_sel(r, al, T);
     const double pa = in_attack ? pm : 1.0, pd = in_attack ? 0.0 : pm;
     return pa * (1.0 - (1.0 - S) * pd) * (1.0 - pr);
 }
@@ -341,17 +346,19 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
     const bool live = (j <= jsil) && (j < K);
     double E[6] = {0, 0, 0, 0, 0, 0};
     unsigned long long dq1 = 0, dq2 = 0;
-    if (live) {
-        const double tau = (double)((long long)j * TS_R) / (double)sr;
-        if (V.slow) {  // some alpha <= 0 (custom nebula): generic path, uniform over the voice
+    const double tau = (double)((long long)j * TS_R) / (double)sr;
+    if (V.slow) {  // some alpha <= 0 (custom nebula): generic path, uniform over the voice
+        if (live) {
 #pragma unroll 1
             for (int e = 0; e < 6; ++e) Es[e][tid] = ts_adsr(tau, e, V, &MT);
 #pragma unroll
             for (int e = 0; e < 6; ++e) E[e] = Es[e][tid];
-        } else {
-#pragma unroll
-            for (int e = 0; e < 6; ++e) E[e] = ts_adsr_fast(tau, e, V, &MT);
         }
+    } else {  // every lane (the warp votes on which powers are needed at all); dead lanes' values are unused
+#pragma unroll
+        for (int e = 0; e < 6; ++e) E[e] = ts_adsr_fast(tau, e, V, &MT);
+    }
+    if (live) {
         const double d1 = fma(V.dq_d[0], E[3], V.dq_f[0]);
         const double d2 = fma(V.dq_d[1], E[5], V.dq_f[1]);
         dq1 = (unsigned long long)__double2ll_rn((d1 - rint(d1)) * 18446744073709551616.0);
