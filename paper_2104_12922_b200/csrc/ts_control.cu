@@ -242,6 +242,7 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
     __shared__ ts_math_tables MT;
     __shared__ unsigned long long scan_sm[64];
     __shared__ unsigned long long acc[4];
+    __shared__ int s_dead;
     __shared__ double2 pitch[TS_CTL_THREADS];
     __shared__ double Es[6][TS_CTL_THREADS];
 
@@ -255,7 +256,25 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
     if (tid < (int)(sizeof(ts_math_tables) / 8))
         reinterpret_cast<double *>(&MT)[tid] = reinterpret_cast<const double *>(&c_math)[tid];
     if (tid < 4) acc[tid] = 0ull;
+    if (c > 0 && tid >= 96 && !full) {
+        // Is this whole chunk past the voice's last audible tick?  Only the duration and the four audible releases
+        // decide that: the last warp maps those five parameters straight from the global tables while the others
+        // stage, and evaluates S4's own predicate at the chunk's first tick.  Dead chunks (55 % of C2's) leave now.
+        const int lane = tid - 96;
+        const int idx = (lane == 0) ? 1 : ((lane == 1) ? 5 : ((lane == 2) ? 10 : ((lane == 3) ? 15 : 25)));
+        const double hv = ts_map((double)rec.u[idx], c_nebula[idx], &c_math);
+        const double Dq = __shfl_sync(0xffffffffu, hv, 0);
+        const double r1 = __shfl_sync(0xffffffffu, hv, 1), r2 = __shfl_sync(0xffffffffu, hv, 2);
+        const double r3 = __shfl_sync(0xffffffffu, hv, 3), r4 = __shfl_sync(0xffffffffu, hv, 4);
+        if (lane == 0) {
+            const long long jj = (long long)c * TS_CTL_IC;
+            s_dead = jj >= K || (((double)(jj * TS_R) / (double)sr) - Dq >= fmax(fmax(r1, r2), fmax(r3, r4)));
+        }
+    } else if (tid == 96) {
+        s_dead = 0;
+    }
     __syncthreads();
+    if (s_dead) return;
     if (tid < TS_NPARAM) {
         const double hv = ts_map((double)rec.u[tid], c_nebula[tid], &MT);
         V.h[tid] = hv;
