@@ -35,13 +35,18 @@ def measured_peak():
 
 
 def ncu_traffic(workload: str):
-    """dram bytes per launch of the audio kernel from the committed ncu --set full capture, if any."""
-    p = os.path.join(ROOT, "profiles", "audio_kernel_dram_bytes.json")
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the audio kernel, from the committed summary of the
+    latest `ncu --set full` capture (profiles/audio_kernel_traffic.csv: workload,bytes), if any."""
+    p = os.path.join(ROOT, "profiles", "audio_kernel_traffic.csv")
     try:
         with open(p) as f:
-            return json.load(f).get(workload)
+            for ln in f:
+                k, _, v = ln.strip().partition(",")
+                if k == workload:
+                    return float(v)
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
@@ -193,32 +198,40 @@ def run_ours(args, wl):
         clocks = clk2.summary()
         clocks["note"] = "timed region shorter than the NVML poll; sampled on the same loop run for 0.3 s"
 
-    # ---- roofline of the dominant kernel (audio): algorithmic bytes = 4 B per output sample
+    # ---- roofline of the dominant kernel (audio): algorithmic bytes = 4 B per output sample (DESIGN.md 5.2)
+    # (a) average launch duration over back-to-back launches (CUDA events on the library's stream around 50 launches
+    #     of each kernel, outputs rotating over the ring); (b) one isolated launch bracketed by its own event pair,
+    #     which adds the ~6 us an empty kernel shows between two events on this box.
+    reps = 50
+    ctl, aud = ts.ts_time_kernels(params[0], sr, seconds, audio_ring, reps)
     ts.ts_set_timing(True)
-    ctl_ms, aud_ms = [], []
-    for i in range(max(5, min(args.steps, 50))):
+    ctl_1, aud_1 = [], []
+    for i in range(10):
         step(i)
         c, a = ts.ts_last_kernel_ms()
-        ctl_ms.append(c)
-        aud_ms.append(a)
+        ctl_1.append(c)
+        aud_1.append(a)
     stats = ts.ts_last_stats()
     launches_per_step = 1 + stats["launches"]
     active_frac = stats["active_samples"] / float(B * N)
     ts.ts_set_timing(False)
     torch.cuda.synchronize()
-    aud = statistics.mean(aud_ms)
-    ctl = statistics.mean(ctl_ms)
     peak, peak_src = measured_peak()
     achieved = out_bytes / (aud * 1e-3) / 1e9
+    traffic = ncu_traffic(wl.name)
     roofline = {"bound": "hbm", "kernel": "ts_audio_kernel<0>", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(wl.name), "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": out_bytes, "audio_kernel_ms": aud, "control_kernel_ms": ctl,
+                "timing": f"CUDA events around {reps} back-to-back launches of each kernel (ts_time_kernels)",
+                "isolated_launch_ms": {"audio": statistics.mean(aud_1), "control": statistics.mean(ctl_1)},
                 "active_sample_fraction": active_frac,
+                "note": "audible samples are issue-bound (~46 SASS instructions each), silent tails are pure stores; "
+                        "see DESIGN.md 5.2 for the issue-slot bound stated beside this HBM one",
                 "whole_step_frac_of_write_roofline": (4.0 * value / world / 1e9) / peak}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32 audio (f64 + Q0.64 integer phase chain)", "data": "synthetic",
+            "dtype": "f32 (audio) + f64 / Q0.64 (control and phase chain)", "data": "synthetic",
             "config": {"workload": f"{wl.name}: B={B} voices x {seconds} s @ {sr} Hz per GPU per step, seed 0, consecutive batch indices "
                                    "through ts_corpus_render (sampler + control + audio per batch)",
                        "l2": f"{nbuf} rotating output buffers of {out_bytes >> 20} MiB (> 126 MB L2 together)"},
@@ -243,9 +256,13 @@ def run_ours(args, wl):
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
-        v, dt = oracle_samples_per_s(wl, wl.B, 2, cores)
+        voices = min(wl.B, 128)
+        _v, dt1 = oracle_samples_per_s(wl, voices, 1, cores)
+        repeats = max(2, min(400, int(15.0 / max(dt1, 1e-3))))           # ~15 s of wall clock on all cores
+        v, dt = oracle_samples_per_s(wl, voices, repeats, cores)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"all {wl.B} voices x {seconds} s, 2 repeats, {dt:.1f} s wall"}
+                                "sample": f"first {voices} voices of the batch x {seconds} s, {repeats} repeats, "
+                                          f"{dt:.1f} s wall on {cores} threads"}
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

@@ -30,7 +30,7 @@ class _Out(C.Structure):
 
 EXPORTS = ["ts_sample_params", "ts_render", "ts_render_host", "ts_corpus_render", "ts_num_samples", "ts_num_ticks", "ts_set_stream",
            "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes", "ts_last_error", "ts_sync", "ts_shutdown",
-           "ts_set_timing", "ts_last_kernel_ms", "ts_last_stats", "ts_debug_noise_u32", "ts_debug_controls",
+           "ts_set_timing", "ts_time_kernels", "ts_last_kernel_ms", "ts_last_stats", "ts_debug_noise_u32", "ts_debug_controls",
            "ts_debug_phase"]
 
 
@@ -65,6 +65,7 @@ def lib():
     L.ts_shutdown.restype = None
     L.ts_set_timing.argtypes = [i32]
     L.ts_last_kernel_ms.argtypes = [vp]
+    L.ts_time_kernels.argtypes = [vp, i32, i32, f64, vp, i32, i32, vp]
     L.ts_last_stats.argtypes = [vp]
     L.ts_debug_noise_u32.argtypes = [vp, u64, i32, vp]
     L.ts_debug_controls.argtypes = [vp, i32, i32, f64, vp]
@@ -144,6 +145,16 @@ def ts_set_timing(enable: bool) -> None:
 def ts_last_kernel_ms():
     ms = (C.c_float * 2)()
     _check(lib().ts_last_kernel_ms(ms))
+    return float(ms[0]), float(ms[1])
+
+
+def ts_time_kernels(params, sr: int, seconds: float, audio_ring, reps: int):
+    """-> (control ms, audio ms) per launch, averaged over `reps` back-to-back launches of each kernel."""
+    p = _dev_params(params)
+    ms = (C.c_float * 2)()
+    _use_current_stream(p.device)
+    _check(lib().ts_time_kernels(C.c_void_p(p.data_ptr()), p.shape[0], sr, float(seconds), C.c_void_p(audio_ring.data_ptr()),
+                                 int(audio_ring.shape[0]), reps, ms))
     return float(ms[0]), float(ms[1])
 
 

@@ -426,6 +426,48 @@ void ts_shutdown(void) {
     S.math_uploaded = false;
 }
 
+int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, float *d_audio_ring, int n_ring, int reps,
+                    float host_ms[2]) {
+    if (!d_params || !d_audio_ring || !host_ms) return fail(TS_ENULL, "NULL argument%s");
+    if (n_ring <= 0 || reps <= 0) return fail(TS_EINVAL, "n_ring and reps must be positive%s");
+    int64_t N;
+    int K;
+    int rc = check_sizes(B, sr, seconds, &N, &K);
+    if (rc) return rc;
+    S.cur = &S.lane[0];
+    rc = prepare_common(sr);
+    if (rc) return rc;
+    if (chunk_voices(B, K) < B) return fail(TS_EINVAL, "ts_time_kernels needs a batch that renders in one voice chunk%s");
+    size_t off_hdr, off_agg;
+    rc = ensure_ws(ws_layout(B, K, &off_hdr, &off_agg));
+    if (rc) return rc;
+    ts_tick *table = reinterpret_cast<ts_tick *>(S.cur->ws);
+    ts_vhdr *hdr = reinterpret_cast<ts_vhdr *>(static_cast<char *>(S.cur->ws) + off_hdr);
+    void *agg = static_cast<char *>(S.cur->ws) + off_agg;
+    for (auto &e : S.ev)
+        if (!e) TS_CUDA(cudaEventCreate(&e));
+    cudaStream_t st = S.cur->stream;
+    TS_CUDA(cudaEventRecord(S.ev[0], st));
+    for (int r = 0; r < reps; ++r) {
+        if (++S.cur->epoch == 0) {
+            TS_CUDA(cudaMemsetAsync(agg, 0, ts_control_agg_bytes(B, K), st));
+            S.cur->epoch = 1;
+        }
+        TS_CUDA(ts_launch_control(d_params, B, sr, N, K, table, hdr, agg, S.cur->epoch, nullptr, nullptr, nullptr, 0, st));
+    }
+    TS_CUDA(cudaEventRecord(S.ev[1], st));
+    for (int r = 0; r < reps; ++r)
+        TS_CUDA(ts_launch_audio(table, hdr, B, N, K, d_audio_ring + (size_t)(r % n_ring) * (size_t)B * (size_t)N, 0, nullptr, st));
+    TS_CUDA(cudaEventRecord(S.ev[2], st));
+    TS_CUDA(cudaEventSynchronize(S.ev[2]));
+    float a = 0.f, b = 0.f;
+    TS_CUDA(cudaEventElapsedTime(&a, S.ev[0], S.ev[1]));
+    TS_CUDA(cudaEventElapsedTime(&b, S.ev[1], S.ev[2]));
+    host_ms[0] = a / (float)reps;
+    host_ms[1] = b / (float)reps;
+    return TS_OK;
+}
+
 int ts_set_timing(int enable) {
     S.timing = enable != 0;
     return TS_OK;
