@@ -68,12 +68,6 @@ __device__ __forceinline__ ts_f2 ts_dup(float c) { return ts_pack(c, c); }
 // has slope up to ~1e5 per cycle at the zero crossings, H4).
 constexpr float SIN_C3 = -0.16666659712791443f, SIN_C5 = 0.008333087898790836f, SIN_C7 = -0.00019811101083178073f,
                 SIN_C9 = 2.6089039693033556e-06f;
-// cos(th) on the same interval as 1 + th^2 r(th^2), r minimax of degree 3: absolute accuracy 1.7e-7 in fp32.  A
-// polynomial instead of MUFU.COS: same issue slots (4 FFMA2 per sample pair), but the XU pipe, which the
-// remaining sin / ex2 / rcp keep busy half the time, gets 25 % less work.
-constexpr float COS_C2 = -0.4999993145465851f, COS_C4 = 0.041663989424705505f, COS_C6 = -0.001385591458529234f,
-                COS_C8 = 2.319407394679729e-05f;
-
 template <int MODE>
 __global__ void __launch_bounds__(TS_AUDIO_THREADS)
 ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ hdr, int B, long long N, int K,
@@ -172,10 +166,9 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
                     Q = ts_fma2(Q, T2, ts_dup(SIN_C3));
                     const ts_f2 SN = ts_fma2(ts_mul2(TH, T2), Q, TH);  // sin(th), th in [-pi/2, pi/2)
                     float ea, eb, da, db;
-                    ts_f2 CS = ts_fma2(T2, ts_dup(COS_C8), ts_dup(COS_C6));
-                    CS = ts_fma2(CS, T2, ts_dup(COS_C4));
-                    CS = ts_fma2(CS, T2, ts_dup(COS_C2));
-                    CS = ts_fma2(CS, T2, ONE);
+                    float tha, thb;
+                    ts_unpack(TH, tha, thb);
+                    const ts_f2 CS = ts_pack(__cosf(tha), __cosf(thb));
                     ts_unpack(ts_mul2(SN, TANH_C), ea, eb);
                     ts_unpack(ts_add2(ts_pack(ts_ex2(ea), ts_ex2(eb)), ONE), da, db);
                     // tanh((pi/2) k sin) = 1 - 2 / (1 + 2^(c sin));  y2 = sigma tanh (1 + s sigma cos) = tanh (sigma + s cos)
