@@ -107,7 +107,7 @@ int ts_last_kernel_ms(float host_ms[2]);
  * control kernel, then `reps` of the audio kernel (output rotating over the n_ring slots of d_audio_ring,
  * [n_ring][B][N] fp32, so that consecutive launches do not rewrite lines still in L2), each group between one pair
  * of CUDA events on the set stream.  host_ms[0] = control, host_ms[1] = audio, milliseconds per launch.
- * Synchronises.  TS_EINVAL if the batch needs more than one voice chunk. */
+ * A batch that ts_render splits into several voice chunks is timed chunk by chunk and summed.  Synchronises. */
 int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, float *d_audio_ring, int n_ring, int reps,
                     float host_ms[2]);
 /* Counters of the LAST ts_render (host): [0] kernels launched, [1] voice chunks,

@@ -437,9 +437,9 @@ int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, flo
     S.cur = &S.lane[0];
     rc = prepare_common(sr);
     if (rc) return rc;
-    if (chunk_voices(B, K) < B) return fail(TS_EINVAL, "ts_time_kernels needs a batch that renders in one voice chunk%s");
+    const int Bc = chunk_voices(B, K);
     size_t off_hdr, off_agg;
-    rc = ensure_ws(ws_layout(B, K, &off_hdr, &off_agg));
+    rc = ensure_ws(ws_layout(Bc, K, &off_hdr, &off_agg));
     if (rc) return rc;
     ts_tick *table = reinterpret_cast<ts_tick *>(S.cur->ws);
     ts_vhdr *hdr = reinterpret_cast<ts_vhdr *>(static_cast<char *>(S.cur->ws) + off_hdr);
@@ -447,22 +447,31 @@ int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, flo
     for (auto &e : S.ev)
         if (!e) TS_CUDA(cudaEventCreate(&e));
     cudaStream_t st = S.cur->stream;
-    TS_CUDA(cudaEventRecord(S.ev[0], st));
-    for (int r = 0; r < reps; ++r) {
-        if (++S.cur->epoch == 0) {
-            TS_CUDA(cudaMemsetAsync(agg, 0, ts_control_agg_bytes(B, K), st));
-            S.cur->epoch = 1;
-        }
-        TS_CUDA(ts_launch_control(d_params, B, sr, N, K, table, hdr, agg, S.cur->epoch, nullptr, nullptr, nullptr, 0, st));
-    }
-    TS_CUDA(cudaEventRecord(S.ev[1], st));
-    for (int r = 0; r < reps; ++r)
-        TS_CUDA(ts_launch_audio(table, hdr, B, N, K, d_audio_ring + (size_t)(r % n_ring) * (size_t)B * (size_t)N, 0, nullptr, st));
-    TS_CUDA(cudaEventRecord(S.ev[2], st));
-    TS_CUDA(cudaEventSynchronize(S.ev[2]));
     float a = 0.f, b = 0.f;
-    TS_CUDA(cudaEventElapsedTime(&a, S.ev[0], S.ev[1]));
-    TS_CUDA(cudaEventElapsedTime(&b, S.ev[1], S.ev[2]));
+    for (int b0 = 0; b0 < B; b0 += Bc) {  // voice chunk by voice chunk, as ts_render launches them
+        const int nb = (B - b0 < Bc) ? (B - b0) : Bc;
+        TS_CUDA(cudaEventRecord(S.ev[0], st));
+        for (int r = 0; r < reps; ++r) {
+            if (++S.cur->epoch == 0) {
+                TS_CUDA(cudaMemsetAsync(agg, 0, ts_control_agg_bytes(Bc, K), st));
+                S.cur->epoch = 1;
+            }
+            TS_CUDA(ts_launch_control(d_params + b0, nb, sr, N, K, table, hdr, agg, S.cur->epoch, nullptr, nullptr, nullptr, 0,
+                                      st));
+        }
+        TS_CUDA(cudaEventRecord(S.ev[1], st));
+        for (int r = 0; r < reps; ++r)
+            TS_CUDA(ts_launch_audio(table, hdr, nb, N, K,
+                                    d_audio_ring + (size_t)(r % n_ring) * (size_t)B * (size_t)N + (size_t)b0 * (size_t)N, 0,
+                                    nullptr, st));
+        TS_CUDA(cudaEventRecord(S.ev[2], st));
+        TS_CUDA(cudaEventSynchronize(S.ev[2]));
+        float x = 0.f, y = 0.f;
+        TS_CUDA(cudaEventElapsedTime(&x, S.ev[0], S.ev[1]));
+        TS_CUDA(cudaEventElapsedTime(&y, S.ev[1], S.ev[2]));
+        a += x;
+        b += y;
+    }
     host_ms[0] = a / (float)reps;
     host_ms[1] = b / (float)reps;
     return TS_OK;
