@@ -86,6 +86,11 @@ int ts_render_host(uint64_t seed, uint64_t batch_index, int B, int sr, double se
 int ts_corpus_render(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds,
                      ts_voice *d_params_ring, float *d_audio_ring, int n_ring);
 
+/* Train/test designation of global voice g ("9 * 1024 samples are designated as train, the next 1024
+ * samples as test, etc.", i.e. one tenth of the corpus): 1 if (g / 1024) % 10 == 9, else 0.  A position in
+ * the corpus, so it is the same for batch size 128 and 1024 (D3).  Host function, no GPU work. */
+int ts_corpus_is_test(uint64_t g);
+
 /* D17: N = llround(sr*seconds);  S5: K = ceil(N/TS_R) + 1 control ticks. */
 int64_t ts_num_samples(int sr, double seconds);
 int64_t ts_num_ticks(int64_t N);

@@ -129,6 +129,12 @@ def adsr(t, A, Dc, S, Rl, alpha, D) -> float:
     return lib().orc_adsr(float(t), float(A), float(Dc), float(S), float(Rl), float(alpha), float(D))
 
 
+def corpus_is_test(g: int) -> bool:
+    L = lib()
+    L.orc_corpus_is_test.argtypes = [C.c_uint64]
+    return bool(L.orc_corpus_is_test(g))
+
+
 def num_ticks(N: int) -> int:
     return lib().orc_num_ticks(N)
 

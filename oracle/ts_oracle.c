@@ -325,3 +325,10 @@ int orc_render_voice(const float u[ORC_NPARAM], const uint32_t noise_key[2], con
 
 /* D17: N = llround(sr * seconds) */
 int64_t orc_num_samples(int sr, double seconds) { return (int64_t)llround((double)sr * seconds); }
+
+/* Train/test designation ("9 * 1024 samples are designated as train, the next 1024 samples as test,
+ * etc."; one tenth of the examples).  Global voice index g -> 1 if test. */
+int orc_corpus_is_test(uint64_t g) {
+    uint64_t block = g / 1024u;      /* blocks of 1024 consecutive sounds */
+    return (block % 10u) == 9u;      /* nine train blocks, then one test block */
+}

@@ -28,7 +28,7 @@ class _Out(C.Structure):
     _fields_ = [("audio", C.c_void_p), ("params_human", C.c_void_p)]
 
 
-EXPORTS = ["ts_sample_params", "ts_render", "ts_render_host", "ts_corpus_render", "ts_num_samples", "ts_num_ticks", "ts_set_stream",
+EXPORTS = ["ts_sample_params", "ts_render", "ts_render_host", "ts_corpus_render", "ts_corpus_is_test", "ts_num_samples", "ts_num_ticks", "ts_set_stream",
            "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes", "ts_last_error", "ts_sync", "ts_shutdown",
            "ts_set_timing", "ts_time_kernels", "ts_last_kernel_ms", "ts_last_stats", "ts_debug_noise_u32", "ts_debug_controls",
            "ts_debug_phase"]
@@ -52,6 +52,7 @@ def lib():
     L.ts_render.argtypes = [vp, i32, i32, f64, _Out]
     L.ts_render_host.argtypes = [u64, u64, i32, i32, f64, vp, vp]
     L.ts_corpus_render.argtypes = [u64, u64, i32, i32, i32, f64, vp, vp, i32]
+    L.ts_corpus_is_test.argtypes = [u64]
     L.ts_num_samples.argtypes = [i32, f64]
     L.ts_num_samples.restype = C.c_int64
     L.ts_num_ticks.argtypes = [C.c_int64]
@@ -98,6 +99,10 @@ def _dev_params(params):
 
 
 # ------------------------------------------------------------------------------------------ host helpers
+def ts_corpus_is_test(g: int) -> bool:
+    return bool(lib().ts_corpus_is_test(g))
+
+
 def ts_num_samples(sr: int, seconds: float) -> int:
     return lib().ts_num_samples(sr, seconds)
 

@@ -98,3 +98,10 @@ def test_c4_edit_holds_the_note_at_the_top():
     u, _ = O.sample_params(0, 0, 4)
     h = O.map_all(W.edit_u(u, wl)[0], W.apply_nebula(O.default_nebula(), wl))
     assert h[0] == 127.0 and h[1] == 30.0 and h[69] == 96.0 and h[72] == 96.0
+
+
+def test_corpus_is_test_matches_oracle_host_only():
+    import oracle as O
+    import paper_2104_12922_b200 as ts
+    for g in list(range(0, 30000, 257)) + [9216, 10239, 10240, 2**40 * 10240 + 9 * 1024 + 5, 2**63 + 9 * 1024]:
+        assert ts.ts_corpus_is_test(g) == O.corpus_is_test(g), g

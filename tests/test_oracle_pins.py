@@ -537,3 +537,19 @@ def test_voice_independence_row_equals_single_render():
     batch = O.render_batch(u, nk, SR, 3000, threads=4)
     for b in (0, 5, 7):
         assert np.array_equal(batch[b], O.render_voice(u[b], nk[b], SR, 3000)["audio"])
+
+
+def test_corpus_train_test_split_follows_p_l102():
+    """9 * 1024 train, the next 1024 test, etc.; one tenth of the examples are test."""
+    assert not any(O.corpus_is_test(g) for g in (0, 1, 1023, 1024, 9 * 1024 - 1))
+    assert all(O.corpus_is_test(g) for g in (9 * 1024, 10 * 1024 - 1, 19 * 1024, 20 * 1024 - 1))
+    assert not O.corpus_is_test(10 * 1024) and not O.corpus_is_test(18 * 1024 + 1023)
+    n = 50 * 10240
+    assert sum(O.corpus_is_test(g) for g in range(0, n, 7)) * 7 == pytest.approx(n / 10, rel=1e-3)
+    # the same sound is train or test whatever the batch size: whole batches of 128 and of 1024 never straddle
+    for B in (128, 1024):
+        for batch in (0, 71, 72, 79, 80, 8, 9, 10):
+            flags = {O.corpus_is_test(batch * B + b) for b in range(B)}
+            assert len(flags) == 1
+    assert O.corpus_is_test(72 * 128) and O.corpus_is_test(79 * 128 + 127) and not O.corpus_is_test(80 * 128)
+    assert O.corpus_is_test(2**40 * 10240 + 9 * 1024 + 5)        # 64-bit indices
