@@ -301,3 +301,32 @@ def test_corpus_render_matches_batch_by_batch(T):
             assert torch.equal(pr[slot], p) and torch.equal(ar[slot], a), (n_ring, slot, i)
     u, nk = O.sample_params(3, first + 8, B)                                 # and against the oracle
     assert_parity(ar[0].cpu().numpy(), O.render_batch(u, nk, sr, N), "corpus")
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_random_nebula_parity(T, seed):
+    """Other hyper-parameter sets (P:L145 'nebula'): curves log-uniform in [0.1, 10] as in the paper's tuning runs
+    (P:L270), random symmetry flags, ranges shrunk at random inside the default ones.  Same table on both sides."""
+    rng = np.random.default_rng(seed)
+    neb_o = O.default_nebula()
+    lo, hi = neb_o["lo"].copy(), neb_o["hi"].copy()
+    a, b = rng.uniform(0, 0.4, 78), rng.uniform(0.6, 1.0, 78)
+    neb_o["lo"], neb_o["hi"] = lo + a * (hi - lo), lo + b * (hi - lo)
+    neb_o["curve"] = np.exp(rng.uniform(np.log(0.1), np.log(10.0), 78))
+    neb_o["symmetric"] = rng.integers(0, 2, 78)
+    neb_o["lo"][[6, 11, 16, 21, 26, 31]] = 0.1          # ADSR alpha stays positive (S4)
+    neb_g = T.ts_default_nebula()
+    for f in ("lo", "hi", "curve", "symmetric"):
+        neb_g[f] = neb_o[f]
+    T.ts_set_nebula(neb_g)
+    try:
+        B, sr, seconds = 12, 44100, 1.2
+        u, nk = O.sample_params(100 + seed, 0, B)
+        N = O.num_samples(sr, seconds)
+        g, human = T.ts_render(to_dev(u, nk), sr, seconds, want_human=True)
+        o = O.render_batch(u, nk, sr, N, neb_o)
+        for v in range(B):
+            assert np.allclose(human[v].cpu().numpy(), O.map_all(u[v], neb_o).astype(np.float32), rtol=3e-7, atol=1e-7)
+        assert_parity(g.cpu().numpy(), o, f"nebula {seed}")
+    finally:
+        T.ts_set_nebula(None)
