@@ -34,10 +34,11 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic(workload: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the audio kernel, from the committed summary of the
-    latest `ncu --set full` capture (profiles/audio_kernel_traffic.csv: workload,bytes), if any."""
-    p = os.path.join(ROOT, "profiles", "audio_kernel_traffic.csv")
+def ncu_value(name: str, workload: str):
+    """A per-launch counter of the audio kernel from the committed summary of the latest `ncu --set full` capture
+    (profiles/<name>.csv: workload,value), if any.  audio_kernel_traffic = dram__bytes_read.sum +
+    dram__bytes_write.sum; audio_kernel_warp_instructions = smsp__inst_executed.sum."""
+    p = os.path.join(ROOT, "profiles", name + ".csv")
     try:
         with open(p) as f:
             for ln in f:
@@ -218,13 +219,21 @@ def run_ours(args, wl):
     torch.cuda.synchronize()
     peak, peak_src = measured_peak()
     achieved = out_bytes / (aud * 1e-3) / 1e9
-    traffic = ncu_traffic(wl.name)
+    traffic = ncu_value("audio_kernel_traffic", wl.name)
+    winst = ncu_value("audio_kernel_warp_instructions", wl.name)
+    sm_hz = 1e6 * float(clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965)
+    issue = None
+    if winst:       # the other bound of this kernel: 148 SMs x 4 schedulers x 1 warp instruction per clock
+        ipeak = 148 * 4 * sm_hz
+        issue = {"bound": "alu", "what": "warp-instruction issue slots", "achieved": winst / (aud * 1e-3), "peak": ipeak,
+                 "unit": "warp-instructions/s", "frac": winst / (aud * 1e-3) / ipeak,
+                 "warp_instructions_per_launch": winst}
     roofline = {"bound": "hbm", "kernel": "ts_audio_kernel<0>", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": out_bytes, "audio_kernel_ms": aud, "control_kernel_ms": ctl,
                 "timing": f"CUDA events around {reps} back-to-back launches of each kernel (ts_time_kernels)",
                 "isolated_launch_ms": {"audio": statistics.mean(aud_1), "control": statistics.mean(ctl_1)},
-                "active_sample_fraction": active_frac,
+                "active_sample_fraction": active_frac, "issue_bound": issue,
                 "note": "audible samples are issue-bound (~46 SASS instructions each), silent tails are pure stores; "
                         "see DESIGN.md 5.2 for the issue-slot bound stated beside this HBM one",
                 "whole_step_frac_of_write_roofline": (4.0 * value / world / 1e9) / peak}
