@@ -86,6 +86,12 @@ int ts_render_host(uint64_t seed, uint64_t batch_index, int B, int sr, double se
 int ts_corpus_render(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds,
                      ts_voice *d_params_ring, float *d_audio_ring, int n_ring);
 
+/* Control-rate rendering on its own (P:L117 control modules at 1/100 of the audio rate; the paper's Fig. 2 workload,
+ * P:L131): the five modulation-mixer rows (S5..S7: six ADSRs, two LFOs, mixer) at the K = ts_num_ticks(N) control
+ * ticks -> d_ctl[B][5][K] fp64, rows M_0 (vco1 pitch), M_1 (vco1 amp), M_2 (vco2 pitch), M_3 (vco2 amp),
+ * M_4 (noise amp).  Ticks after the voice has gone silent for good are written as 0.  No audio is rendered. */
+int ts_render_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl);
+
 /* Train/test designation of global voice g ("9 * 1024 samples are designated as train, the next 1024
  * samples as test, etc.", i.e. one tenth of the corpus): 1 if (g / 1024) % 10 == 9, else 0.  A position in
  * the corpus, so it is the same for batch size 128 and 1024 (D3).  Host function, no GPU work. */
@@ -123,9 +129,7 @@ int ts_last_stats(int64_t host_stats[3]);
 /* Debug exports used only by the parity tests. */
 /* S12: words n0..n0+count-1 of the noise stream of `key` (host array of 2) -> d_out[count]. */
 int ts_debug_noise_u32(const uint32_t host_key[2], uint64_t n0, int count, uint32_t *d_out);
-/* S5..S7: modulation-mixer rows at the control ticks -> d_ctl[B][5][K] fp64.  Rows 0 and 2 (pitch)
- * are M_0, M_2; rows 1, 3, 4 are the amplitude rows M_1, M_3, M_4.  Ticks after the voice has gone
- * silent for good (S4 release over on all four audible envelopes) are written as 0. */
+/* Same as ts_render_controls (kept under its original name for the parity tests). */
 int ts_debug_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl);
 /* S9: phase of VCO `vco` (1 or 2) at every sample, cycles in [0,1) -> d_phase[B][N] fp64. */
 int ts_debug_phase(const ts_voice *d_params, int B, int sr, double seconds, int vco, double *d_phase);

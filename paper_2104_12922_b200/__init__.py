@@ -7,4 +7,4 @@ There is no CPU fallback: importing `binding` fails loudly if the library has no
 from .binding import (NPARAM, R, NEBULA_DTYPE, TsynthError, lib, lib_path, ts_sample_params, ts_render,  # noqa: F401
                       ts_render_host, ts_corpus_render, ts_corpus_is_test, ts_num_samples, ts_num_ticks, ts_set_stream, ts_default_nebula,
                       ts_set_nebula, ts_workspace_bytes, ts_sync, ts_shutdown, ts_set_timing, ts_time_kernels,
-                      ts_last_kernel_ms, ts_last_stats, ts_debug_noise_u32, ts_debug_controls, ts_debug_phase)
+                      ts_last_kernel_ms, ts_last_stats, ts_debug_noise_u32, ts_debug_controls, ts_render_controls, ts_debug_phase)

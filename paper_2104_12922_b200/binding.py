@@ -30,7 +30,7 @@ class _Out(C.Structure):
 
 EXPORTS = ["ts_sample_params", "ts_render", "ts_render_host", "ts_corpus_render", "ts_corpus_is_test", "ts_num_samples", "ts_num_ticks", "ts_set_stream",
            "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes", "ts_last_error", "ts_sync", "ts_shutdown",
-           "ts_set_timing", "ts_time_kernels", "ts_last_kernel_ms", "ts_last_stats", "ts_debug_noise_u32", "ts_debug_controls",
+           "ts_set_timing", "ts_time_kernels", "ts_last_kernel_ms", "ts_last_stats", "ts_debug_noise_u32", "ts_debug_controls", "ts_render_controls",
            "ts_debug_phase"]
 
 
@@ -70,6 +70,7 @@ def lib():
     L.ts_last_stats.argtypes = [vp]
     L.ts_debug_noise_u32.argtypes = [vp, u64, i32, vp]
     L.ts_debug_controls.argtypes = [vp, i32, i32, f64, vp]
+    L.ts_render_controls.argtypes = [vp, i32, i32, f64, vp]
     L.ts_debug_phase.argtypes = [vp, i32, i32, f64, i32, vp]
     _lib = L
     return L
@@ -249,6 +250,18 @@ def ts_debug_controls(params, sr: int, seconds: float):
     out = torch.empty((B, 5, K), dtype=torch.float64, device=p.device)
     _use_current_stream(p.device)
     _check(lib().ts_debug_controls(C.c_void_p(p.data_ptr()), B, sr, float(seconds), C.c_void_p(out.data_ptr())))
+    return out
+
+
+def ts_render_controls(params, sr: int, seconds: float):
+    """-> CUDA float64 tensor [B, 5, K]: the modulation-mixer rows at the control ticks (S5..S7)."""
+    torch = _torch()
+    p = _dev_params(params)
+    B = p.shape[0]
+    K = ts_num_ticks(ts_num_samples(sr, seconds))
+    out = torch.empty((B, 5, K), dtype=torch.float64, device=p.device)
+    _use_current_stream(p.device)
+    _check(lib().ts_render_controls(C.c_void_p(p.data_ptr()), B, sr, float(seconds), C.c_void_p(out.data_ptr())))
     return out
 
 

@@ -506,6 +506,9 @@ int ts_debug_controls(const ts_voice *d_params, int B, int sr, double seconds, d
     if (!d_params || !d_ctl) return fail(TS_ENULL, "NULL argument%s");
     return render_impl(d_params, B, sr, seconds, nullptr, nullptr, 3, d_ctl);
 }
+int ts_render_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl) {
+    return ts_debug_controls(d_params, B, sr, seconds, d_ctl);
+}
 int ts_debug_phase(const ts_voice *d_params, int B, int sr, double seconds, int vco, double *d_phase) {
     if (!d_params || !d_phase) return fail(TS_ENULL, "NULL argument%s");
     if (vco != 1 && vco != 2) return fail(TS_EINVAL, "vco must be 1 or 2%s");

@@ -330,3 +330,16 @@ def test_random_nebula_parity(T, seed):
         assert_parity(g.cpu().numpy(), o, f"nebula {seed}")
     finally:
         T.ts_set_nebula(None)
+
+
+def test_render_controls_c2_sampled_voices(T):
+    """The control-rate call on its own (Fig. 2 workload) at C2 size against the oracle's mixer rows."""
+    wl, neb, u, nk, dev = setup_workload(T, "C2")
+    ctl = T.ts_render_controls(dev, wl.sr, wl.seconds).cpu().numpy()
+    assert ctl.shape == (wl.B, 5, O.num_ticks(wl.N))
+    for b in range(0, wl.B, 9):
+        E, L, M = O.controls(O.map_all(u[b], neb), wl.sr, wl.N)
+        nz = np.flatnonzero(np.any(M != 0.0, axis=0))
+        last = nz[-1] + 1 if nz.size else 0
+        assert np.max(np.abs(ctl[b] - M)) < 1e-12, b
+        assert not np.any(ctl[b][:, last:]), b
