@@ -343,3 +343,28 @@ def test_render_controls_c2_sampled_voices(T):
         last = nz[-1] + 1 if nz.size else 0
         assert np.max(np.abs(ctl[b] - M)) < 1e-12, b
         assert not np.any(ctl[b][:, last:]), b
+
+
+def test_c3_streaming_protocol_100_batches(T):
+    """BASELINE.json configs[2]: 1024 voices x 4 s rendered over 100 consecutive batch indices, here in the bench's
+    launch configuration (ts_corpus_render, two alternating output slots); the last two batches against the oracle
+    on sampled voices, records bit-exact."""
+    import torch
+    wl = W.WORKLOADS["C3"]
+    T.ts_set_nebula(None)
+    pr = torch.empty((2, wl.B, 80), device="cuda")
+    ar = torch.empty((2, wl.B, wl.N), device="cuda")
+    T.ts_corpus_render(wl.seed, 0, wl.batches, wl.sr, wl.seconds, pr, ar)
+    torch.cuda.synchronize()
+    voices = np.arange(5, 1024, 64)
+    neb = O.default_nebula()
+    for batch in (wl.batches - 2, wl.batches - 1):
+        slot = batch % 2
+        u, nk = O.sample_params(wl.seed, batch, wl.B)
+        rec = pr[slot].cpu().numpy()
+        assert np.array_equal(rec[:, :78].view(np.uint32), u.view(np.uint32))
+        assert np.array_equal(np.ascontiguousarray(rec[:, 78:]).view(np.uint32), nk)
+        g = ar[slot][voices.tolist()].cpu().numpy()
+        o = O.render_batch(u[voices], nk[voices], wl.sr, wl.N, neb)
+        assert_parity(g, o, f"C3 stream[{batch}]")
+        assert T.ts_corpus_is_test(batch * wl.B) == O.corpus_is_test(batch * wl.B)
