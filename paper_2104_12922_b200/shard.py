@@ -19,6 +19,9 @@ def batch_index(step: int, rank: int, world_size: int, first: int = 0) -> int:
 def init(backend: str):
     import torch.distributed as dist
     rank, local_rank, ws = world()
+    if backend == "nccl":          # one process per GPU: bind the device before NCCL picks one
+        import torch
+        torch.cuda.set_device(local_rank)
     if ws > 1 and not dist.is_initialized():
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         os.environ.setdefault("MASTER_PORT", "29511")
