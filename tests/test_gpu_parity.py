@@ -298,7 +298,8 @@ def test_corpus_render_matches_batch_by_batch(T):
             i = max(k for k in range(n_batches) if k % n_ring == slot)      # the last batch written to this slot
             p = T.ts_sample_params(3, first + i, B)
             a = T.ts_render(p, sr, seconds)
-            assert torch.equal(pr[slot], p) and torch.equal(ar[slot], a), (n_ring, slot, i)
+            assert torch.equal(pr[slot].view(torch.int32), p.view(torch.int32)), (n_ring, slot, i)   # keys may be NaN patterns
+            assert torch.equal(ar[slot], a), (n_ring, slot, i)
     u, nk = O.sample_params(3, first + 8, B)                                 # and against the oracle
     assert_parity(ar[0].cpu().numpy(), O.render_batch(u, nk, sr, N), "corpus")
 
