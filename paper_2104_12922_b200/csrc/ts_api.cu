@@ -114,6 +114,16 @@ bool nebula_supported(int sr) {
     return inc * TS_R < 262000.0;
 }
 
+// Does the active nebula leave a long exactly-silent tail in a buffer of `seconds`?  Every voice is silent after
+// duration + the longest release of the four audible envelopes (H6); if even the longest such voice leaves a fifth of
+// the buffer silent, the audio kernel lets its audible CTAs write the tails (ts_audio.cu, TAIL = 1).
+int tails_expected(double seconds) {
+    const ts_range *n = S.nebula;
+    auto hi = [&](int i) { return fmax(n[i].lo, n[i].hi); };
+    const double t_end = hi(1) + fmax(fmax(hi(5), hi(10)), fmax(hi(15), hi(25)));
+    return t_end < 0.8 * seconds;
+}
+
 int ensure_ws(size_t bytes) {
     if (bytes <= S.cur->ws_bytes) return TS_OK;
     if (S.cur->ws) cudaFree(S.cur->ws);
@@ -226,7 +236,7 @@ int render_impl(const ts_voice *d_params, int B, int sr, double seconds, float *
             TS_CUDA(cudaStreamWaitEvent(ast, S.cur->ctl_done, 0));
         }
         if (mode != 3) {
-            TS_CUDA(ts_launch_audio(table, hdr, nb, N, K, audio ? audio + (size_t)b0 * N : nullptr, mode,
+            TS_CUDA(ts_launch_audio(table, hdr, nb, N, K, audio ? audio + (size_t)b0 * N : nullptr, mode, tails_expected(seconds),
                                     (mode == 1 || mode == 2) ? dbg + (size_t)b0 * N : nullptr, ast));
             ++launches;
         }
@@ -465,7 +475,7 @@ int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, flo
         for (int r = 0; r < reps; ++r)
             TS_CUDA(ts_launch_audio(table, hdr, nb, N, K,
                                     d_audio_ring + (size_t)(r % n_ring) * (size_t)B * (size_t)N + (size_t)b0 * (size_t)N, 0,
-                                    nullptr, st));
+                                    tails_expected(seconds), nullptr, st));
         TS_CUDA(cudaEventRecord(S.ev[2], st));
         TS_CUDA(cudaEventSynchronize(S.ev[2]));
         float x = 0.f, y = 0.f;

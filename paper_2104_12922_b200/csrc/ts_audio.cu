@@ -9,7 +9,7 @@
 // so no thread ever waits for another.  Everything downstream of the reduced phase is fp32.
 // The tile is staged in shared memory (conflict-free STS.128) and leaves the SM as ONE bulk
 // asynchronous copy (cp.async.bulk, the TMA engine), i.e. fully coalesced 10 KB writes.
-// Tiles past the voice's last audible sample are written as zeros without any arithmetic.
+// Tiles past the voice's last audible sample are written as zeros without any arithmetic, by the voice's audible CTAs.
 #include "ts_common.cuh"
 
 namespace {
@@ -28,10 +28,12 @@ __device__ __forceinline__ float ts_rcp(float x) {
     return y;
 }
 
-__device__ __forceinline__ void ts_bulk_store(void *gdst, const void *ssrc, uint32_t bytes) {
-    const uint32_t s = (uint32_t)__cvta_generic_to_shared(ssrc);
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(s), "r"(bytes)
+__device__ __forceinline__ void ts_bulk_issue(void *gdst, uint32_t ssrc, uint32_t bytes) {  // TMA engine (UBLKCP)
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(ssrc), "r"(bytes)
                  : "memory");
+}
+__device__ __forceinline__ void ts_bulk_store(void *gdst, const void *ssrc, uint32_t bytes) {
+    ts_bulk_issue(gdst, (uint32_t)__cvta_generic_to_shared(ssrc), bytes);
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
@@ -68,11 +70,14 @@ __device__ __forceinline__ ts_f2 ts_dup(float c) { return ts_pack(c, c); }
 // has slope up to ~1e5 per cycle at the zero crossings, H4).
 constexpr float SIN_C3 = -0.16666659712791443f, SIN_C5 = 0.008333087898790836f, SIN_C7 = -0.00019811101083178073f,
                 SIN_C9 = 2.6089039693033556e-06f;
-template <int MODE>
+// TAIL = 1: the silent tails are written by the audible CTAs (below); TAIL = 0: every silent tile is written by a CTA of
+// its own (better when few tiles are silent: no zero buffer, more L1 left for the control table).
+template <int MODE, int TAIL>
 __global__ void __launch_bounds__(TS_AUDIO_THREADS)
 ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ hdr, int B, long long N, int K,
                 float *__restrict__ audio, double *__restrict__ dbg_phase, int aligned, uint32_t one_bits) {
     __shared__ __align__(128) float4 stage[TS_TILE / 4];
+    __shared__ __align__(128) float4 zero[(MODE == 0 && TAIL) ? TS_TILE / 4 : 4];  // source of the tail's zero-fill bulk copies
 
     const int voice = blockIdx.x % B;  // time-major grid: the audible (expensive) tiles are dispatched first
     const long long tile = blockIdx.x / B;
@@ -83,7 +88,7 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
     const int count = (rem < TS_TILE) ? (int)rem : TS_TILE;  // samples of this tile inside the buffer
     float *row = audio + (size_t)voice * N + n_tile0;
 
-    if (MODE == 0 && n_tile0 >= hd.n_act) {  // silent tile: exact zeros (S4 release over; pin P9)
+    if (MODE == 0 && !TAIL && n_tile0 >= hd.n_act) {  // silent tile: exact zeros (S4 release over; pin P9)
         if (aligned) {
             float4 *r4 = reinterpret_cast<float4 *>(row);
             for (int i = tid; i < count / 4; i += TS_AUDIO_THREADS) r4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -91,6 +96,39 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
             for (int i = tid; i < count; i += TS_AUDIO_THREADS) row[i] = 0.f;
         }
         return;
+    }
+    if (MODE == 0 && TAIL) {
+        // Samples [n_act, N) are exactly 0 (S4 release over; pin P9).  The silent tiles of a voice are not rendered by
+        // CTAs of their own: audible tile t of a voice with A audible tiles writes the silent tiles A + t, A + t + A, ...
+        // as asynchronous bulk copies of a zero buffer (TMA engine), issued BEFORE its arithmetic, so that the stores
+        // of the tails overlap the issue-bound arithmetic of the audible part instead of following it.
+        const long long T = (N + TS_TILE - 1) / TS_TILE;
+        long long A = ((long long)hd.n_act + TS_TILE - 1) / TS_TILE;
+        if (A < 1) A = 1;  // a voice with no audible sample: tile 0 renders zeros and owns the whole tail
+        if (tile >= A) return;
+        float *vrow = audio + (size_t)voice * N;
+        if (A + tile >= T) {
+            // no silent tile falls to this CTA
+        } else if (aligned) {
+#pragma unroll
+            for (int g = 0; g < TS_RUN / 4; ++g) zero[tid * (TS_RUN / 4) + g] = make_float4(0.f, 0.f, 0.f, 0.f);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> async proxy
+            __syncthreads();
+            if ((tid & 31) == 0) {  // lane 0 of each warp issues every fourth copy
+                const uint32_t zs = (uint32_t)__cvta_generic_to_shared(zero);
+                for (long long tz = A + tile + (tid >> 5) * A; tz < T; tz += (TS_AUDIO_THREADS / 32) * A) {
+                    const long long rz = N - tz * TS_TILE;
+                    ts_bulk_issue(vrow + tz * TS_TILE, zs, (rz < TS_TILE) ? (uint32_t)rz * 4u : (uint32_t)TS_TILE * 4u);
+                }
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            }
+        } else {
+            for (long long tz = A + tile; tz < T; tz += A) {
+                const long long rz = N - tz * TS_TILE;
+                const int cz = (rz < TS_TILE) ? (int)rz : TS_TILE;
+                for (int i = tid; i < cz; i += TS_AUDIO_THREADS) vrow[tz * TS_TILE + i] = 0.f;
+            }
+        }
     }
 
     const long long r = tile * TS_AUDIO_THREADS + tid;  // run index inside the voice
@@ -202,6 +240,7 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> async proxy
         __syncthreads();
         if (tid == 0) ts_bulk_store(row, stage, (uint32_t)count * 4u);
+        else if (TAIL && (tid & 31) == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // zero buffer still being read
     } else {
         __syncthreads();
         const float *sf = reinterpret_cast<const float *>(stage);
@@ -212,16 +251,18 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
 }  // namespace
 
 cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, float *audio,
-                            int mode, double *dbg_phase, cudaStream_t st) {
+                            int mode, int tails, double *dbg_phase, cudaStream_t st) {
     const int64_t tiles = (N + TS_TILE - 1) / TS_TILE;
     const int64_t grid = tiles * B;
     if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = (N % 4 == 0) && ((reinterpret_cast<uintptr_t>(audio) & 15u) == 0);
-    if (mode == 0)
-        ts_audio_kernel<0><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u);
+    if (mode == 0 && tails)
+        ts_audio_kernel<0, 1><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u);
+    else if (mode == 0)
+        ts_audio_kernel<0, 0><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u);
     else if (mode == 1)
-        ts_audio_kernel<1><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, 0, 0x3f800000u);
+        ts_audio_kernel<1, 0><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, 0, 0x3f800000u);
     else
-        ts_audio_kernel<2><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, 0, 0x3f800000u);
+        ts_audio_kernel<2, 0><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, 0, 0x3f800000u);
     return cudaGetLastError();
 }

@@ -68,6 +68,7 @@ size_t ts_control_agg_bytes(int B, int K);  // look-back slots; must be zero bef
 cudaError_t ts_launch_control(const ts_voice *d_params, int B, int sr, int64_t N, int K, ts_tick *table,
                               ts_vhdr *hdr, void *agg, unsigned int epoch, float *params_human, double *dbg_ctl,
                               unsigned long long *d_active, int full, cudaStream_t st);
-// mode 0: audio; mode 1 / 2: write the phase of VCO 1 / 2 (fp64 cycles) to dbg_phase instead
+// mode 0: audio; mode 1 / 2: write the phase of VCO 1 / 2 (fp64 cycles) to dbg_phase instead.
+// tails != 0: long silent tails are expected (nebula + buffer length), let the audible CTAs write them asynchronously
 cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, float *audio,
-                            int mode, double *dbg_phase, cudaStream_t st);
+                            int mode, int tails, double *dbg_phase, cudaStream_t st);
