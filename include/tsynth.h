@@ -13,7 +13,9 @@
  *     return without synchronising, except ts_render_host(), ts_sync() and ts_shutdown().
  *   - Return value 0 = TS_OK, negative = error; ts_last_error() gives the text.  No exceptions,
  *     no abort(), nothing printed.
- *   - Not thread-safe: one host thread drives one library instance (one GPU per process).
+ *   - Not thread-safe: one host thread drives one library instance (one GPU per process).  The library state (nebula,
+ *     workspaces, internal streams) is one process-wide singleton: one nebula at a time, one device per process, which
+ *     is what one-process-per-GPU launches (torchrun) need.
  */
 #ifndef TSYNTH_H
 #define TSYNTH_H
@@ -70,11 +72,24 @@ int ts_sample_params(uint64_t seed, uint64_t batch_index, int B, ts_voice *d_par
  * oscillator increment beyond the supported 2^18/TS_R cycles per sample at this sr). */
 int ts_render(const ts_voice *d_params, int B, int sr, double seconds, ts_out out);
 
+/* Output sample formats.  The path computes in fp32 (fp64 / Q0.64 for the phase chain) whatever the format; TS_F16 and
+ * TS_BF16 round the finished fp32 sample once (round to nearest even) when it is stored, which halves the path's only
+ * HBM traffic and the device->host bytes of an end-to-end call ("faster to render ... than to
+ * download").  |sample| <= 1.125 (S11), so fp16 never overflows. */
+enum { TS_F32 = 0, TS_F16 = 1, TS_BF16 = 2 };
+
+/* ts_render with the output format chosen per call: d_audio is [B][N] of float, __half or __nv_bfloat16 (device). */
+int ts_render_fmt(const ts_voice *d_params, int B, int sr, double seconds, int fmt, void *d_audio,
+                  float *d_params_human);
+
 /* Convenience end-to-end call with HOST buffers: ts_sample_params + ts_render on the device, then
  * device->host copies of audio ([B][N] fp32) and, if host_params is not NULL, of the ts_voice
  * records.  Synchronises.  Device staging memory belongs to the library workspace. */
 int ts_render_host(uint64_t seed, uint64_t batch_index, int B, int sr, double seconds,
                    float *host_audio, ts_voice *host_params);
+/* The same with the output format chosen per call (host_audio: [B][N] of float / half / bfloat16). */
+int ts_render_host_fmt(uint64_t seed, uint64_t batch_index, int B, int sr, double seconds, int fmt,
+                       void *host_audio, ts_voice *host_params);
 
 /* Streaming corpus generation ("generated on the fly from a batch index"; BASELINE.json configs[2]):
  * batches first_batch .. first_batch + n_batches - 1 of B voices each, batch i sampled and rendered into ring slot
@@ -86,11 +101,59 @@ int ts_render_host(uint64_t seed, uint64_t batch_index, int B, int sr, double se
 int ts_corpus_render(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds,
                      ts_voice *d_params_ring, float *d_audio_ring, int n_ring);
 
+/* ts_corpus_render with the output format chosen per call (d_audio_ring: [n_ring][B][N] of float / half / bfloat16). */
+int ts_corpus_render_fmt(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds, int fmt,
+                         ts_voice *d_params_ring, void *d_audio_ring, int n_ring);
+
+/* Streaming corpus ITERATOR ("generated on the fly", P:L98 sounds paired with their
+ * parameters, P:L102 train/test blocks).  ts_corpus_open() fixes the corpus (seed, B, sr, seconds, format), the caller's
+ * ring of n_ring >= 2 output slots and the first batch index, and starts rendering n_ring - 1 batches ahead on the
+ * library's internal streams.  Each ts_corpus_next() hands out the next batch: the slot's device pointers, the batch
+ * index, the global index of its first voice (g = batch_index * B) and the train/test designation of its first and last
+ * voice (equal whenever B divides 1024; a batch of 1024-aligned voices never straddles a block).  The call makes the set stream wait
+ * for that batch (no host synchronisation) and re-arms the slot handed out by the PREVIOUS call with the batch
+ * n_ring - 1 ahead, ordered after everything the caller has queued on the set stream so far: consume a batch on the set
+ * stream before asking for the next one.  ts_corpus_close() drains the internal streams. */
+typedef struct {
+    uint64_t seed;
+    int B, sr;
+    double seconds;
+    int fmt;                 /* TS_F32 / TS_F16 / TS_BF16 */
+    int n_ring;              /* >= 2 */
+    void *d_audio_ring;      /* [n_ring][B][N] in fmt (device, caller-owned) */
+    ts_voice *d_params_ring; /* [n_ring][B] records (device, caller-owned) */
+} ts_corpus_cfg;
+typedef struct {
+    void *d_audio;           /* [B][N] in the corpus format */
+    ts_voice *d_params;      /* [B] records: normalised parameters + noise keys */
+    uint64_t batch_index;
+    uint64_t first_voice;    /* global voice index of row 0 */
+    int is_test_first, is_test_last; /* ts_corpus_is_test of the first and the last voice of the batch */
+    int slot;
+} ts_corpus_batch;
+int ts_corpus_open(const ts_corpus_cfg *host_cfg, uint64_t first_batch);
+int ts_corpus_next(ts_corpus_batch *host_out);
+int ts_corpus_close(void);
+
 /* Control-rate rendering on its own (P:L117 control modules at 1/100 of the audio rate; the paper's Fig. 2 workload,
  * P:L131): the five modulation-mixer rows (S5..S7: six ADSRs, two LFOs, mixer) at the K = ts_num_ticks(N) control
  * ticks -> d_ctl[B][5][K] fp64, rows M_0 (vco1 pitch), M_1 (vco1 amp), M_2 (vco2 pitch), M_3 (vco2 amp),
- * M_4 (noise amp).  Ticks after the voice has gone silent for good are written as 0.  No audio is rendered. */
+ * M_4 (noise amp).  Ticks after the voice has gone silent for good are written as 0.  No audio is rendered and nothing
+ * of the oscillator stage runs (no interval sums, no phase scan, no control table). */
 int ts_render_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl);
+/* The same with the tick spacing chosen per call: one tick every R >= 1 samples (control rate sr / R, reading D2 with R
+ * in place of 100); K = ts_num_ticks_r(N, R) = ceil(N / R) + 1.  R = 1 is the audio-rate-control mode of SURVEY 8(f)
+ * item 3 (upsampling is then the identity, pin P7): every ADSR / LFO / mixer value is evaluated at every sample. */
+int ts_render_controls_r(const ts_voice *d_params, int B, int sr, double seconds, int R, double *d_ctl);
+int64_t ts_num_ticks_r(int64_t N, int R);
+
+/* Maximum mean discrepancy of two sets of n embeddings of dimension d with the l1 distance as the core distance
+ * (Eq. 2 at P:L230; "1/nn" there is read as 1/n^2, reading D25; the paper's setting is n = 1000, d = 512,
+ * P:L257):  MMD(X, Y) = (1/n^2) sum_{i,j} [ 2 |x_i - y_j|_1 - |x_i - x_j|_1 - |y_i - y_j|_1 ].
+ * d_x, d_y: [n][d] fp32 row-major (device).  d_out (device, 4 doubles): [0] MMD, [1] sum_ij |x_i - y_j|_1,
+ * [2] sum_ij |x_i - x_j|_1, [3] sum_ij |y_i - y_j|_1.  Differences and per-pair sums are fp32, sums over pairs fp64,
+ * reduced in a fixed order (bitwise reproducible).  Errors: TS_ENULL, TS_EINVAL (n <= 0, d <= 0, n > 65535). */
+int ts_mmd_l1(const float *d_x, const float *d_y, int n, int d, double *d_out);
 
 /* Train/test designation of global voice g ("9 * 1024 samples are designated as train, the next 1024
  * samples as test, etc.", i.e. one tenth of the corpus): 1 if (g / 1024) % 10 == 9, else 0.  A position in
@@ -106,7 +169,7 @@ int ts_default_nebula(ts_range host_out78[TS_NPARAM]); /* host copy of the built
 int ts_set_nebula(const ts_range *host_in78);      /* host table; NULL restores the default        */
 size_t ts_workspace_bytes(int B, int sr, double seconds); /* device bytes ts_render will hold      */
 const char *ts_last_error(void);                   /* host string, owned by the library            */
-int ts_sync(void);                                 /* cudaStreamSynchronize on the set stream      */
+int ts_sync(void);                                 /* cudaStreamSynchronize on the set stream; TS_ECUDA if a kernel raised the device error flag */
 void ts_shutdown(void);                            /* frees the workspace                          */
 
 /* Per-kernel device times of the LAST ts_render when timing is enabled (CUDA events on the set
@@ -121,6 +184,10 @@ int ts_last_kernel_ms(float host_ms[2]);
  * A batch that ts_render splits into several voice chunks is timed chunk by chunk and summed.  Synchronises. */
 int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, float *d_audio_ring, int n_ring, int reps,
                     float host_ms[2]);
+/* Measurement aid: average device time of a store-only kernel (128-bit stores of zeros over d_dst[0 .. bytes)), `reps`
+ * launches between one pair of CUDA events on the set stream -> *host_ms per launch.  What a pure store stream reaches on
+ * this GPU, quoted beside the copy peak the roofline uses.  Synchronises. */
+int ts_time_fill(void *d_dst, size_t bytes, int reps, float *host_ms);
 /* Counters of the LAST ts_render (host): [0] kernels launched, [1] voice chunks,
  * [2] audio samples in the active (non-silent) prefix summed over voices (counted only while timing is
  * enabled with ts_set_timing; valid after ts_sync). */
@@ -129,7 +196,8 @@ int ts_last_stats(int64_t host_stats[3]);
 /* Debug exports used only by the parity tests. */
 /* S12: words n0..n0+count-1 of the noise stream of `key` (host array of 2) -> d_out[count]. */
 int ts_debug_noise_u32(const uint32_t host_key[2], uint64_t n0, int count, uint32_t *d_out);
-/* Same as ts_render_controls (kept under its original name for the parity tests). */
+/* The five modulation-mixer rows as the AUDIO path computes them (same launch as ts_render up to the control table,
+ * every tick evaluated) -> d_ctl[B][5][K] fp64. */
 int ts_debug_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl);
 /* S9: phase of VCO `vco` (1 or 2) at every sample, cycles in [0,1) -> d_phase[B][N] fp64. */
 int ts_debug_phase(const ts_voice *d_params, int B, int sr, double seconds, int vco, double *d_phase);

@@ -28,10 +28,23 @@ class _Out(C.Structure):
     _fields_ = [("audio", C.c_void_p), ("params_human", C.c_void_p)]
 
 
-EXPORTS = ["ts_sample_params", "ts_render", "ts_render_host", "ts_corpus_render", "ts_corpus_is_test", "ts_num_samples", "ts_num_ticks", "ts_set_stream",
-           "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes", "ts_last_error", "ts_sync", "ts_shutdown",
-           "ts_set_timing", "ts_time_kernels", "ts_last_kernel_ms", "ts_last_stats", "ts_debug_noise_u32", "ts_debug_controls", "ts_render_controls",
+EXPORTS = ["ts_sample_params", "ts_render", "ts_render_fmt", "ts_render_host", "ts_render_host_fmt", "ts_corpus_render",
+           "ts_corpus_render_fmt", "ts_corpus_open", "ts_corpus_next", "ts_corpus_close", "ts_corpus_is_test", "ts_num_samples",
+           "ts_num_ticks", "ts_num_ticks_r", "ts_set_stream", "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes",
+           "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_time_kernels", "ts_time_fill", "ts_last_kernel_ms",
+           "ts_last_stats", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_debug_noise_u32", "ts_debug_controls",
            "ts_debug_phase"]
+TS_F32, TS_F16, TS_BF16 = 0, 1, 2
+
+
+class _CorpusCfg(C.Structure):
+    _fields_ = [("seed", C.c_uint64), ("B", C.c_int), ("sr", C.c_int), ("seconds", C.c_double), ("fmt", C.c_int),
+                ("n_ring", C.c_int), ("d_audio_ring", C.c_void_p), ("d_params_ring", C.c_void_p)]
+
+
+class _CorpusBatch(C.Structure):
+    _fields_ = [("d_audio", C.c_void_p), ("d_params", C.c_void_p), ("batch_index", C.c_uint64), ("first_voice", C.c_uint64),
+                ("is_test_first", C.c_int), ("is_test_last", C.c_int), ("slot", C.c_int)]
 
 
 def lib_path() -> str:
@@ -50,8 +63,18 @@ def lib():
     vp, u64, i32, f64 = C.c_void_p, C.c_uint64, C.c_int, C.c_double
     L.ts_sample_params.argtypes = [u64, u64, i32, vp]
     L.ts_render.argtypes = [vp, i32, i32, f64, _Out]
+    L.ts_render_fmt.argtypes = [vp, i32, i32, f64, i32, vp, vp]
     L.ts_render_host.argtypes = [u64, u64, i32, i32, f64, vp, vp]
+    L.ts_render_host_fmt.argtypes = [u64, u64, i32, i32, f64, i32, vp, vp]
     L.ts_corpus_render.argtypes = [u64, u64, i32, i32, i32, f64, vp, vp, i32]
+    L.ts_corpus_render_fmt.argtypes = [u64, u64, i32, i32, i32, f64, i32, vp, vp, i32]
+    L.ts_corpus_open.argtypes = [C.POINTER(_CorpusCfg), u64]
+    L.ts_corpus_next.argtypes = [C.POINTER(_CorpusBatch)]
+    L.ts_num_ticks_r.argtypes = [C.c_int64, i32]
+    L.ts_num_ticks_r.restype = C.c_int64
+    L.ts_time_fill.argtypes = [vp, C.c_size_t, i32, vp]
+    L.ts_render_controls_r.argtypes = [vp, i32, i32, f64, i32, vp]
+    L.ts_mmd_l1.argtypes = [vp, vp, i32, i32, vp]
     L.ts_corpus_is_test.argtypes = [u64]
     L.ts_num_samples.argtypes = [i32, f64]
     L.ts_num_samples.restype = C.c_int64
@@ -231,6 +254,129 @@ def ts_corpus_render(seed: int, first_batch: int, n_batches: int, sr: int, secon
     _check(lib().ts_corpus_render(seed, first_batch, n_batches, B, sr, float(seconds), C.c_void_p(params_ring.data_ptr()),
                                   C.c_void_p(audio_ring.data_ptr()), R_))
     return audio_ring
+
+
+def _fmt_dtype(fmt: int):
+    torch = _torch()
+    return {TS_F32: torch.float32, TS_F16: torch.float16, TS_BF16: torch.bfloat16}[fmt]
+
+
+def ts_num_ticks_r(N: int, R: int) -> int:
+    return lib().ts_num_ticks_r(N, R)
+
+
+def ts_render_fmt(params, sr: int, seconds: float, fmt: int, out=None):
+    """ts_render with the output format chosen per call -> audio [B, N] in float32 / float16 / bfloat16."""
+    torch = _torch()
+    p = _dev_params(params)
+    B = p.shape[0]
+    N = ts_num_samples(sr, seconds)
+    dt = _fmt_dtype(fmt)
+    if out is None:
+        out = torch.empty((B, N), dtype=dt, device=p.device)
+    elif not (out.is_cuda and out.dtype == dt and out.is_contiguous() and tuple(out.shape) == (B, N)):
+        raise TsynthError("out must be a contiguous CUDA tensor [B, N] of the chosen format")
+    _use_current_stream(p.device)
+    _check(lib().ts_render_fmt(C.c_void_p(p.data_ptr()), B, sr, float(seconds), fmt, C.c_void_p(out.data_ptr()), None))
+    return out
+
+
+def ts_render_host_fmt(seed: int, batch_index: int, B: int, sr: int, seconds: float, fmt: int, host_audio=None, host_params=None):
+    """End to end with HOST buffers in the chosen format (pinned torch CPU tensors): sample + render + D2H."""
+    torch = _torch()
+    N = ts_num_samples(sr, seconds)
+    if host_audio is None:
+        host_audio = torch.empty((B, N), dtype=_fmt_dtype(fmt), pin_memory=True)
+    pp = host_params.data_ptr() if host_params is not None else None
+    _use_current_stream(torch.device("cuda", torch.cuda.current_device()))
+    _check(lib().ts_render_host_fmt(seed, batch_index, B, sr, float(seconds), fmt, C.c_void_p(host_audio.data_ptr()),
+                                    C.c_void_p(pp) if pp else None))
+    return host_audio
+
+
+def ts_corpus_render_fmt(seed: int, first_batch: int, n_batches: int, sr: int, seconds: float, fmt: int, params_ring, audio_ring):
+    """ts_corpus_render with the output format chosen per call; audio_ring [R, B, N] in that format."""
+    R_, B = int(params_ring.shape[0]), int(params_ring.shape[1])
+    N = ts_num_samples(sr, seconds)
+    if not (audio_ring.is_cuda and audio_ring.dtype == _fmt_dtype(fmt) and audio_ring.is_contiguous()
+            and tuple(audio_ring.shape) == (R_, B, N)):
+        raise TsynthError("audio_ring must be a contiguous CUDA tensor [R, B, N] of the chosen format")
+    _use_current_stream(params_ring.device)
+    _check(lib().ts_corpus_render_fmt(seed, first_batch, n_batches, B, sr, float(seconds), fmt, C.c_void_p(params_ring.data_ptr()),
+                                      C.c_void_p(audio_ring.data_ptr()), R_))
+    return audio_ring
+
+
+_corpus_rings = None
+
+
+def ts_corpus_open(seed: int, first_batch: int, sr: int, seconds: float, fmt: int, params_ring, audio_ring) -> None:
+    """Opens the streaming iterator over the caller's rings: params_ring [R, B, 80] fp32, audio_ring [R, B, N] in fmt."""
+    global _corpus_rings
+    R_, B = int(params_ring.shape[0]), int(params_ring.shape[1])
+    N = ts_num_samples(sr, seconds)
+    if not (params_ring.is_cuda and params_ring.is_contiguous() and params_ring.shape[2] == REC_FLOATS):
+        raise TsynthError("params_ring must be a contiguous CUDA float32 tensor [R, B, 80]")
+    if not (audio_ring.is_cuda and audio_ring.dtype == _fmt_dtype(fmt) and audio_ring.is_contiguous()
+            and tuple(audio_ring.shape) == (R_, B, N)):
+        raise TsynthError("audio_ring must be a contiguous CUDA tensor [R, B, N] of the chosen format")
+    cfg = _CorpusCfg(seed, B, sr, float(seconds), fmt, R_, audio_ring.data_ptr(), params_ring.data_ptr())
+    _use_current_stream(params_ring.device)
+    _check(lib().ts_corpus_open(C.byref(cfg), first_batch))
+    _corpus_rings = (params_ring, audio_ring)
+
+
+def ts_corpus_next():
+    """-> dict(audio [B, N] view of the ring slot, params [B, 80] view, batch_index, first_voice, is_test_first,
+    is_test_last, slot).  The current torch stream waits for the batch; consume it there before the next call."""
+    if _corpus_rings is None:
+        raise TsynthError("no corpus iterator is open")
+    params_ring, audio_ring = _corpus_rings
+    b = _CorpusBatch()
+    _use_current_stream(params_ring.device)
+    _check(lib().ts_corpus_next(C.byref(b)))
+    assert b.d_audio == audio_ring[b.slot].data_ptr() and b.d_params == params_ring[b.slot].data_ptr()
+    return {"audio": audio_ring[b.slot], "params": params_ring[b.slot], "batch_index": int(b.batch_index),
+            "first_voice": int(b.first_voice), "is_test_first": bool(b.is_test_first), "is_test_last": bool(b.is_test_last),
+            "slot": int(b.slot)}
+
+
+def ts_corpus_close() -> None:
+    global _corpus_rings
+    _check(lib().ts_corpus_close())
+    _corpus_rings = None
+
+
+def ts_time_fill(buf, reps: int) -> float:
+    """-> ms per launch of a store-only fill of `buf` (a CUDA tensor)."""
+    ms = C.c_float()
+    _use_current_stream(buf.device)
+    _check(lib().ts_time_fill(C.c_void_p(buf.data_ptr()), buf.numel() * buf.element_size(), reps, C.byref(ms)))
+    return float(ms.value)
+
+
+def ts_render_controls_r(params, sr: int, seconds: float, R: int):
+    """-> CUDA float64 tensor [B, 5, K_R]: the modulation-mixer rows with one control tick every R samples."""
+    torch = _torch()
+    p = _dev_params(params)
+    B = p.shape[0]
+    K = ts_num_ticks_r(ts_num_samples(sr, seconds), R)
+    out = torch.empty((B, 5, K), dtype=torch.float64, device=p.device)
+    _use_current_stream(p.device)
+    _check(lib().ts_render_controls_r(C.c_void_p(p.data_ptr()), B, sr, float(seconds), R, C.c_void_p(out.data_ptr())))
+    return out
+
+
+def ts_mmd_l1(x, y):
+    """x, y: CUDA float32 [n, d] -> CUDA float64 [4]: MMD (Eq. 2), sum |x_i - y_j|_1, sum |x_i - x_j|_1, sum |y_i - y_j|_1."""
+    torch = _torch()
+    if not (x.is_cuda and y.is_cuda and x.dtype == torch.float32 and y.dtype == torch.float32 and x.is_contiguous()
+            and y.is_contiguous() and x.dim() == 2 and tuple(x.shape) == tuple(y.shape)):
+        raise TsynthError("x and y must be contiguous CUDA float32 tensors of the same shape [n, d]")
+    out = torch.empty(4, dtype=torch.float64, device=x.device)
+    _use_current_stream(x.device)
+    _check(lib().ts_mmd_l1(C.c_void_p(x.data_ptr()), C.c_void_p(y.data_ptr()), int(x.shape[0]), int(x.shape[1]), C.c_void_p(out.data_ptr())))
+    return out
 
 
 def ts_debug_noise_u32(key, n0: int, count: int, device="cuda:0"):

@@ -1,5 +1,6 @@
 // ts_api.cu -- the C-ABI of include/tsynth.h: argument checks, the nebula, the workspace (control tables
-// sized to stay L2-resident), voice chunking and kernel launches.  No arithmetic of the method lives here.
+// sized to stay L2-resident), voice chunking, kernel launches and the streaming iterator.  No arithmetic of the
+// method lives here.
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
@@ -9,23 +10,37 @@
 namespace {
 
 // A lane = a workspace with the stream(s) that use it, so that two batches can be in flight at once.
-// Lane 0 serves ts_render / ts_render_host on the caller's stream.  Lanes 1 and 2 serve ts_corpus_render: they
-// share one HIGH-priority stream for the sampler and the (latency-bound) control kernel and one LOW-priority
-// stream for the (issue-bound) audio kernel, so that the control stage of batch i+1 is dispatched into the SMs
-// while the audio stage of batch i still runs and fills the issue slots it leaves idle.
+// Lane 0 serves ts_render / ts_render_host on the caller's stream.  Lanes 1 and 2 serve the streaming calls: they
+// share one HIGH-priority stream for the (latency-bound) setup and control kernels and one LOW-priority stream for
+// the (issue-bound) audio kernel, so that the control stage of batch i+1 is dispatched into the SMs while the audio
+// stage of batch i still runs and fills the issue slots it leaves idle.
 struct ts_lane {
     cudaStream_t stream = nullptr;
     void *ws = nullptr;
     size_t ws_bytes = 0;
-    unsigned int epoch = 0;  // look-back flag value of the latest control launch on this workspace
+    int lay_B = 0, lay_K = 0;  // layout the look-back slots were last cleared for
+    size_t lay_off = 0;
+    unsigned int epoch = 0;    // look-back flag value of the latest control launch on this workspace
     unsigned long long *d_active = nullptr;
     unsigned long long *h_active = nullptr;  // pinned
-    // lanes 1, 2 (ts_corpus_render): the audio kernel goes to its own low-priority stream
+    unsigned int *d_err = nullptr;           // raised by a kernel whose look-back wait gave up
+    unsigned int *h_err = nullptr;           // pinned
+    // lanes 1, 2: the audio kernel goes to its own low-priority stream
     cudaStream_t audio_stream = nullptr;
     cudaEvent_t ctl_done = nullptr, aud_done = nullptr;
     bool aud_pending = false;  // aud_done was recorded after the latest audio kernel that reads this workspace
 };
 constexpr int TS_LANES = 3;
+constexpr int TS_MAX_RING = 64;
+
+struct ts_corpus_state {  // the streaming iterator (ts_corpus_open / next / close)
+    bool open = false;
+    ts_corpus_cfg cfg;
+    int64_t N = 0;
+    uint64_t next_out = 0, next_render = 0;  // batch indices
+    cudaEvent_t ready[TS_MAX_RING] = {};     // slot rendered
+    cudaEvent_t consumed = nullptr;          // the caller's stream has passed the previous hand-out
+};
 
 struct ts_state {
     char err[512] = "";
@@ -36,15 +51,19 @@ struct ts_state {
     ts_lane lane[TS_LANES];
     ts_lane *cur = &lane[0];
     cudaEvent_t fork = nullptr;
-    cudaStream_t hi = nullptr, lo = nullptr;  // ts_corpus_render's internal streams
+    cudaStream_t hi = nullptr, lo = nullptr;  // the streaming calls' internal streams
+    uint64_t stream_count = 0;                // batches issued on the internal streams (picks lane 1 / 2)
     // host staging for ts_render_host
     void *stage = nullptr;
     size_t stage_bytes = 0;
+    double *mmd_ws = nullptr;
+    size_t mmd_ws_count = 0;
     // timing / stats
     bool timing = false;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
     float ms[2] = {0.f, 0.f};
     int64_t stats[3] = {0, 0, 0};
+    ts_corpus_state corpus;
 };
 ts_state S;
 
@@ -65,6 +84,9 @@ int cuda_fail(cudaError_t e, const char *where) {
         cudaError_t e__ = (call);                          \
         if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
     } while (0)
+
+bool fmt_ok(int fmt) { return fmt == TS_F32 || fmt == TS_F16 || fmt == TS_BF16; }
+size_t fmt_bytes(int fmt) { return (fmt == TS_F32) ? 4 : 2; }
 
 void default_nebula(ts_range *n) {  // table S2 (D6, D8); ranges from BASELINE.json configs[0]
     auto set = [&](int i, double lo, double hi, double c, int sym) { n[i] = ts_range{lo, hi, c, sym}; };
@@ -105,6 +127,7 @@ void ensure_nebula() {
 
 // The audio kernel reads frac(phase) out of the fp64 mantissa after adding 1.5*2^19, which needs the
 // phase advance over one control interval to stay below 2^18 cycles (1.5*2^19 +- 2^18 keeps its exponent).
+// ts_set_nebula keeps the weight rows non-negative, so |M_d| <= 1 and pitch <= midi + tune + |depth|.
 bool nebula_supported(int sr) {
     const ts_range *n = S.nebula;
     auto hi = [&](int i) { return fmax(n[i].lo, n[i].hi); };
@@ -124,22 +147,6 @@ int tails_expected(double seconds) {
     return t_end < 0.8 * seconds;
 }
 
-int ensure_ws(size_t bytes) {
-    if (bytes <= S.cur->ws_bytes) return TS_OK;
-    if (S.cur->ws) cudaFree(S.cur->ws);
-    S.cur->ws = nullptr;
-    S.cur->ws_bytes = 0;
-    if (cudaMalloc(&S.cur->ws, bytes) != cudaSuccess) {
-        cudaGetLastError();
-        return fail(TS_ENOMEM, "workspace allocation failed%s");
-    }
-    S.cur->ws_bytes = bytes;
-    // look-back flags must never equal a future epoch: start from zeros and restart the epoch count
-    if (cudaMemsetAsync(S.cur->ws, 0, bytes, S.cur->stream) != cudaSuccess) return cuda_fail(cudaGetLastError(), "cudaMemsetAsync");
-    S.cur->epoch = 0;
-    return TS_OK;
-}
-
 int chunk_voices(int B, int K) {
     size_t per = (size_t)K * sizeof(ts_tick);
     size_t c = TS_TABLE_BUDGET / per;
@@ -147,21 +154,62 @@ int chunk_voices(int B, int K) {
     if (c > (size_t)B) c = (size_t)B;
     return (int)c;
 }
-size_t ws_layout(int Bc, int K, size_t *off_hdr, size_t *off_agg = nullptr) {
-    size_t table = ((size_t)Bc * K * sizeof(ts_tick) + 255) & ~(size_t)255;
-    if (off_hdr) *off_hdr = table;
-    size_t agg = table + (((size_t)Bc * sizeof(ts_vhdr) + 255) & ~(size_t)255);
-    if (off_agg) *off_agg = agg;
-    return agg + ((ts_control_agg_bytes(Bc, K) + 255) & ~(size_t)255);
+struct ws_layout_t {
+    size_t off_hdr, off_vc, off_agg, agg_bytes, total;
+};
+ws_layout_t ws_layout(int Bc, int K, bool table) {
+    auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    ws_layout_t L;
+    L.off_hdr = table ? up((size_t)Bc * K * sizeof(ts_tick)) : 0;
+    L.off_vc = L.off_hdr + up((size_t)Bc * sizeof(ts_vhdr));
+    L.off_agg = L.off_vc + up((size_t)Bc * sizeof(ts_voice_consts));
+    L.agg_bytes = ts_control_agg_bytes(Bc, K);
+    L.total = L.off_agg + up(L.agg_bytes);
+    return L;
 }
 
-int check_sizes(int B, int sr, double seconds, int64_t *N, int *K) {
-    if (B <= 0 || sr <= 0 || !(seconds > 0.0)) return fail(TS_EINVAL, "B, sr and seconds must be positive%s");
+// Grows the workspace if needed and makes sure the look-back slots of THIS layout hold no flag a future epoch could
+// equal: the slots sit at an offset that depends on (Bc, K), so after a layout change they alias bytes that held
+// table or header data; they are cleared and the epoch count restarts whenever the layout changes.
+int ensure_ws(const ws_layout_t &L, int Bc, int K) {
+    ts_lane &ln = *S.cur;
+    if (L.total > ln.ws_bytes) {
+        if (ln.ws) {
+            cudaStreamSynchronize(ln.stream);
+            if (ln.audio_stream) cudaStreamSynchronize(ln.audio_stream);
+            cudaFree(ln.ws);
+        }
+        ln.ws = nullptr;
+        ln.ws_bytes = 0;
+        ln.aud_pending = false;
+        if (cudaMalloc(&ln.ws, L.total) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(TS_ENOMEM, "workspace allocation failed%s");
+        }
+        ln.ws_bytes = L.total;
+        ln.lay_B = ln.lay_K = 0;
+    }
+    if (ln.lay_B != Bc || ln.lay_K != K || ln.lay_off != L.off_agg) {
+        if (ln.aud_pending) {  // an audio kernel may still read the old layout's table
+            TS_CUDA(cudaStreamWaitEvent(ln.stream, ln.aud_done, 0));
+            ln.aud_pending = false;
+        }
+        TS_CUDA(cudaMemsetAsync(static_cast<char *>(ln.ws) + L.off_agg, 0, L.agg_bytes, ln.stream));
+        ln.epoch = 0;
+        ln.lay_B = Bc;
+        ln.lay_K = K;
+        ln.lay_off = L.off_agg;
+    }
+    return TS_OK;
+}
+
+int check_sizes(int B, int sr, double seconds, int64_t *N, int *K, int R = TS_R) {
+    if (B <= 0 || sr <= 0 || !(seconds > 0.0) || R <= 0) return fail(TS_EINVAL, "B, sr, seconds and R must be positive%s");
     const double ns = (double)sr * seconds;
     if (!(ns < 2.0e9)) return fail(TS_EINVAL, "sr*seconds too large%s");
     *N = ts_num_samples(sr, seconds);
     if (*N <= 0) return fail(TS_EINVAL, "zero samples%s");
-    *K = (int)ts_num_ticks(*N);
+    *K = (int)ts_num_ticks_r(*N, R);
     if ((double)B * (double)*N > 9.0e18 / 8) return fail(TS_EINVAL, "B*N overflows%s");
     return TS_OK;
 }
@@ -177,30 +225,58 @@ int prepare_common(int sr) {
         TS_CUDA(ts_upload_math_tables(S.cur->stream));
         S.math_uploaded = true;
     }
-    if (!S.cur->d_active) {
-        TS_CUDA(cudaMalloc(&S.cur->d_active, sizeof(unsigned long long)));
-        TS_CUDA(cudaMallocHost(&S.cur->h_active, sizeof(unsigned long long)));
-        *S.cur->h_active = 0;
+    return TS_OK;
+}
+int prepare_lane() {
+    ts_lane &ln = *S.cur;
+    if (!ln.d_active) {
+        TS_CUDA(cudaMalloc(&ln.d_active, sizeof(unsigned long long)));
+        TS_CUDA(cudaMallocHost(&ln.h_active, sizeof(unsigned long long)));
+        *ln.h_active = 0;
+        TS_CUDA(cudaMalloc(&ln.d_err, sizeof(unsigned int)));
+        TS_CUDA(cudaMallocHost(&ln.h_err, sizeof(unsigned int)));
+        *ln.h_err = 0;
+        TS_CUDA(cudaMemsetAsync(ln.d_err, 0, sizeof(unsigned int), ln.stream));
     }
     return TS_OK;
 }
 
-// mode 0: audio (+ optional params_human); 1/2: debug phase of VCO 1/2; 3: debug controls only
-int render_impl(const ts_voice *d_params, int B, int sr, double seconds, float *audio, float *params_human, int mode,
-                double *dbg) {
+struct sample_spec {  // the fused sampler of the streaming path: draw the records in the setup kernel
+    bool on;
+    uint64_t seed, g0;
+};
+
+// mode 0: audio (+ optional params_human); 1/2: debug phase of VCO 1/2; 3: debug controls of the audio path;
+// mode 4: control-rate rendering on its own (no oscillator stage; tick spacing R)
+int render_impl(ts_voice *d_params, sample_spec smp, int B, int sr, double seconds, int fmt, void *audio, float *params_human,
+                int mode, double *dbg, int R = TS_R) {
     int64_t N;
     int K;
-    int rc = check_sizes(B, sr, seconds, &N, &K);
+    int rc = check_sizes(B, sr, seconds, &N, &K, R);
     if (rc) return rc;
-    rc = prepare_common(sr);
+    if (!fmt_ok(fmt)) return fail(TS_EINVAL, "unknown output format%s");
+    if (S.cur == &S.lane[0]) {  // the streaming calls upload on the caller's stream before they fork
+        rc = prepare_common(sr);
+        if (rc) return rc;
+    }
+    rc = prepare_lane();
     if (rc) return rc;
-    const int Bc = chunk_voices(B, K);
-    size_t off_hdr, off_agg;
-    rc = ensure_ws(ws_layout(Bc, K, &off_hdr, &off_agg));
+    const bool with_table = (mode != 4);
+    int Bc = with_table ? chunk_voices(B, K) : B;
+    if (!with_table) {  // control-rate rendering: bound the look-back slots and the per-launch grid
+        const size_t cap = ((size_t)1 << 25) / (size_t)K;
+        if ((size_t)Bc > cap) Bc = cap ? (int)cap : 1;
+    }
+    const ws_layout_t L = ws_layout(Bc, K, with_table);
+    rc = ensure_ws(L, Bc, K);
     if (rc) return rc;
-    ts_tick *table = reinterpret_cast<ts_tick *>(S.cur->ws);
-    ts_vhdr *hdr = reinterpret_cast<ts_vhdr *>(static_cast<char *>(S.cur->ws) + off_hdr);
-    void *agg = static_cast<char *>(S.cur->ws) + off_agg;
+    ts_lane &ln = *S.cur;
+    char *ws = static_cast<char *>(ln.ws);
+    ts_tick *table = reinterpret_cast<ts_tick *>(ws);
+    ts_vhdr *hdr = reinterpret_cast<ts_vhdr *>(ws + L.off_hdr);
+    ts_voice_consts *vc = reinterpret_cast<ts_voice_consts *>(ws + L.off_vc);
+    void *agg = ws + L.off_agg;
+    const size_t es = fmt_bytes(fmt);
 
     if (S.timing && mode == 0)
         for (auto &e : S.ev)
@@ -208,44 +284,45 @@ int render_impl(const ts_voice *d_params, int B, int sr, double seconds, float *
     S.ms[0] = S.ms[1] = 0.f;
     int64_t launches = 0, chunks = 0;
     const bool want_stats = S.timing;  // the active-sample count costs a memset and a copy per call
-    if (want_stats) TS_CUDA(cudaMemsetAsync(S.cur->d_active, 0, sizeof(unsigned long long), S.cur->stream));
-    if (mode == 3) TS_CUDA(cudaMemsetAsync(dbg, 0, (size_t)B * 5 * K * sizeof(double), S.cur->stream));
+    if (want_stats) TS_CUDA(cudaMemsetAsync(ln.d_active, 0, sizeof(unsigned long long), ln.stream));
 
     for (int b0 = 0; b0 < B; b0 += Bc) {
         const int nb = (B - b0 < Bc) ? (B - b0) : Bc;
         const bool timed = S.timing && mode == 0;
-        if (timed) TS_CUDA(cudaEventRecord(S.ev[0], S.cur->stream));
-        if (S.cur->aud_pending) {  // the audio kernel still reading this workspace's table goes first
-            TS_CUDA(cudaStreamWaitEvent(S.cur->stream, S.cur->aud_done, 0));
-            S.cur->aud_pending = false;
+        if (timed) TS_CUDA(cudaEventRecord(S.ev[0], ln.stream));
+        if (ln.aud_pending) {  // the audio kernel still reading this workspace's table goes first
+            TS_CUDA(cudaStreamWaitEvent(ln.stream, ln.aud_done, 0));
+            ln.aud_pending = false;
         }
-        if (++S.cur->epoch == 0) {  // wrapped after 2^32 launches: clear the flags and start over
-            TS_CUDA(cudaMemsetAsync(agg, 0, ts_control_agg_bytes(Bc, K), S.cur->stream));
-            S.cur->epoch = 1;
+        if (++ln.epoch == 0) {  // wrapped after 2^32 launches: clear the flags and start over
+            TS_CUDA(cudaMemsetAsync(agg, 0, L.agg_bytes, ln.stream));
+            ln.epoch = 1;
         }
-        TS_CUDA(ts_launch_control(d_params + b0, nb, sr, N, K, table, hdr, agg, S.cur->epoch,
-                                  params_human ? params_human + (size_t)b0 * TS_NPARAM : nullptr,
-                                  mode == 3 ? dbg + (size_t)b0 * 5 * K : nullptr, want_stats ? S.cur->d_active : nullptr,
-                                  (mode == 1 || mode == 2) ? 1 : 0, S.cur->stream));
-        ++launches;
-        if (timed) TS_CUDA(cudaEventRecord(S.ev[1], S.cur->stream));
-        cudaStream_t ast = S.cur->stream;
-        if (S.cur->audio_stream && mode == 0) {  // hand over to the audio stream
-            ast = S.cur->audio_stream;
-            TS_CUDA(cudaEventRecord(S.cur->ctl_done, S.cur->stream));
-            TS_CUDA(cudaStreamWaitEvent(ast, S.cur->ctl_done, 0));
+        TS_CUDA(ts_launch_setup(d_params + b0, smp.on ? 1 : 0, smp.seed, smp.g0 + (uint64_t)b0, nb, sr, R, N, K, vc, hdr,
+                                params_human ? params_human + (size_t)b0 * TS_NPARAM : nullptr,
+                                want_stats ? ln.d_active : nullptr, (mode == 1 || mode == 2 || mode == 3) ? 1 : 0, ln.stream));
+        TS_CUDA(ts_launch_control(vc, nb, sr, R, N, K, table, agg, ln.epoch,
+                                  (mode == 3 || mode == 4) ? dbg + (size_t)b0 * 5 * K : nullptr, with_table ? 1 : 0, ln.d_err,
+                                  ln.stream));
+        launches += 2;
+        if (timed) TS_CUDA(cudaEventRecord(S.ev[1], ln.stream));
+        cudaStream_t ast = ln.stream;
+        if (ln.audio_stream && mode == 0) {  // hand over to the audio stream
+            ast = ln.audio_stream;
+            TS_CUDA(cudaEventRecord(ln.ctl_done, ln.stream));
+            TS_CUDA(cudaStreamWaitEvent(ast, ln.ctl_done, 0));
         }
-        if (mode != 3) {
-            TS_CUDA(ts_launch_audio(table, hdr, nb, N, K, audio ? audio + (size_t)b0 * N : nullptr, mode, tails_expected(seconds),
-                                    (mode == 1 || mode == 2) ? dbg + (size_t)b0 * N : nullptr, ast));
+        if (mode <= 2) {
+            TS_CUDA(ts_launch_audio(table, hdr, nb, N, K, audio ? static_cast<char *>(audio) + (size_t)b0 * N * es : nullptr, fmt,
+                                    mode, tails_expected(seconds), (mode == 1 || mode == 2) ? dbg + (size_t)b0 * N : nullptr, ast));
             ++launches;
         }
-        if (ast != S.cur->stream) {  // the next control launch on this workspace will wait for this audio kernel
-            TS_CUDA(cudaEventRecord(S.cur->aud_done, ast));
-            S.cur->aud_pending = true;
+        if (ast != ln.stream) {  // the next control launch on this workspace will wait for this audio kernel
+            TS_CUDA(cudaEventRecord(ln.aud_done, ast));
+            ln.aud_pending = true;
         }
         if (timed) {
-            TS_CUDA(cudaEventRecord(S.ev[2], S.cur->stream));
+            TS_CUDA(cudaEventRecord(S.ev[2], ln.stream));
             TS_CUDA(cudaEventSynchronize(S.ev[2]));
             float a = 0.f, b = 0.f;
             TS_CUDA(cudaEventElapsedTime(&a, S.ev[0], S.ev[1]));
@@ -256,10 +333,57 @@ int render_impl(const ts_voice *d_params, int B, int sr, double seconds, float *
         ++chunks;
     }
     if (want_stats)
-        TS_CUDA(cudaMemcpyAsync(S.cur->h_active, S.cur->d_active, sizeof(unsigned long long), cudaMemcpyDeviceToHost,
-                                S.cur->stream));
+        TS_CUDA(cudaMemcpyAsync(ln.h_active, ln.d_active, sizeof(unsigned long long), cudaMemcpyDeviceToHost, ln.stream));
     S.stats[0] = launches;
     S.stats[1] = chunks;
+    return TS_OK;
+}
+
+int ensure_streams() {
+    if (S.fork) return TS_OK;
+    int lo_p = 0, hi_p = 0;
+    TS_CUDA(cudaDeviceGetStreamPriorityRange(&lo_p, &hi_p));  // numerically lower = higher priority
+    TS_CUDA(cudaStreamCreateWithPriority(&S.hi, cudaStreamNonBlocking, hi_p));
+    TS_CUDA(cudaStreamCreateWithPriority(&S.lo, cudaStreamNonBlocking, lo_p));
+    for (int l = 1; l < TS_LANES; ++l) {
+        S.lane[l].stream = S.hi;
+        S.lane[l].audio_stream = S.lo;
+        TS_CUDA(cudaEventCreateWithFlags(&S.lane[l].ctl_done, cudaEventDisableTiming));
+        TS_CUDA(cudaEventCreateWithFlags(&S.lane[l].aud_done, cudaEventDisableTiming));
+    }
+    TS_CUDA(cudaEventCreateWithFlags(&S.fork, cudaEventDisableTiming));
+    return TS_OK;
+}
+
+// Both internal streams start after everything already queued on the caller's stream.
+int fork_streams() {
+    TS_CUDA(cudaEventRecord(S.fork, S.lane[0].stream));
+    TS_CUDA(cudaStreamWaitEvent(S.hi, S.fork, 0));
+    TS_CUDA(cudaStreamWaitEvent(S.lo, S.fork, 0));
+    return TS_OK;
+}
+
+// One batch of the streaming path on the internal streams: records drawn and set up on `hi`, audio on `lo`.
+int stream_batch(uint64_t seed, uint64_t batch, int B, int sr, double seconds, int fmt, ts_voice *p, void *a) {
+    ts_lane &L = S.lane[1 + (int)(S.stream_count++ & 1)];
+    S.cur = &L;
+    const bool timing = S.timing;
+    S.timing = false;  // per-kernel events would serialise the streams
+    const int rc = render_impl(p, sample_spec{true, seed, batch * (uint64_t)B}, B, sr, seconds, fmt, a, nullptr, 0, nullptr);
+    S.timing = timing;
+    S.cur = &S.lane[0];
+    return rc;
+}
+
+int corpus_issue(uint64_t batch) {  // render `batch` into its slot and record the slot's ready event on `lo`
+    ts_corpus_state &C = S.corpus;
+    const int slot = (int)(batch % (uint64_t)C.cfg.n_ring);
+    const size_t es = fmt_bytes(C.cfg.fmt);
+    const int rc = stream_batch(C.cfg.seed, batch, C.cfg.B, C.cfg.sr, C.cfg.seconds, C.cfg.fmt,
+                                C.cfg.d_params_ring + (size_t)slot * (size_t)C.cfg.B,
+                                static_cast<char *>(C.cfg.d_audio_ring) + (size_t)slot * (size_t)C.cfg.B * (size_t)C.N * es);
+    if (rc) return rc;
+    TS_CUDA(cudaEventRecord(C.ready[slot], S.lo));
     return TS_OK;
 }
 
@@ -271,6 +395,7 @@ int ts_corpus_is_test(uint64_t g) { return (g / 1024u) % 10u == 9u; }
 
 int64_t ts_num_samples(int sr, double seconds) { return (int64_t)llround((double)sr * seconds); }
 int64_t ts_num_ticks(int64_t N) { return (N + TS_R - 1) / TS_R + 1; }
+int64_t ts_num_ticks_r(int64_t N, int R) { return (R > 0) ? (N + R - 1) / R + 1 : 0; }
 
 int ts_sample_params(uint64_t seed, uint64_t batch_index, int B, ts_voice *d_params) {
     if (!d_params) return fail(TS_ENULL, "d_params is NULL%s");
@@ -279,21 +404,29 @@ int ts_sample_params(uint64_t seed, uint64_t batch_index, int B, ts_voice *d_par
     return TS_OK;
 }
 
+int ts_render_fmt(const ts_voice *d_params, int B, int sr, double seconds, int fmt, void *d_audio, float *d_params_human) {
+    if (!d_params) return fail(TS_ENULL, "d_params is NULL%s");
+    if (!d_audio) return fail(TS_ENULL, "audio is NULL%s");
+    return render_impl(const_cast<ts_voice *>(d_params), sample_spec{false, 0, 0}, B, sr, seconds, fmt, d_audio, d_params_human, 0,
+                       nullptr);
+}
+
 int ts_render(const ts_voice *d_params, int B, int sr, double seconds, ts_out out) {
     if (!d_params) return fail(TS_ENULL, "d_params is NULL%s");
     if (!out.audio) return fail(TS_ENULL, "out.audio is NULL%s");
-    return render_impl(d_params, B, sr, seconds, out.audio, out.params_human, 0, nullptr);
+    return ts_render_fmt(d_params, B, sr, seconds, TS_F32, out.audio, out.params_human);
 }
 
-int ts_render_host(uint64_t seed, uint64_t batch_index, int B, int sr, double seconds, float *host_audio,
-                   ts_voice *host_params) {
+int ts_render_host_fmt(uint64_t seed, uint64_t batch_index, int B, int sr, double seconds, int fmt, void *host_audio,
+                       ts_voice *host_params) {
     if (!host_audio) return fail(TS_ENULL, "host_audio is NULL%s");
     int64_t N;
     int K;
     int rc = check_sizes(B, sr, seconds, &N, &K);
     if (rc) return rc;
+    if (!fmt_ok(fmt)) return fail(TS_EINVAL, "unknown output format%s");
     const size_t pbytes = ((size_t)B * sizeof(ts_voice) + 255) & ~(size_t)255;
-    const size_t abytes = (size_t)B * N * sizeof(float);
+    const size_t abytes = (size_t)B * N * fmt_bytes(fmt);
     if (pbytes + abytes > S.stage_bytes) {
         if (S.stage) cudaFree(S.stage);
         S.stage = nullptr;
@@ -305,70 +438,125 @@ int ts_render_host(uint64_t seed, uint64_t batch_index, int B, int sr, double se
         S.stage_bytes = pbytes + abytes;
     }
     ts_voice *d_params = static_cast<ts_voice *>(S.stage);
-    float *d_audio = reinterpret_cast<float *>(static_cast<char *>(S.stage) + pbytes);
-    rc = ts_sample_params(seed, batch_index, B, d_params);
-    if (rc) return rc;
-    rc = render_impl(d_params, B, sr, seconds, d_audio, nullptr, 0, nullptr);
+    void *d_audio = static_cast<char *>(S.stage) + pbytes;
+    rc = render_impl(d_params, sample_spec{true, seed, batch_index * (uint64_t)B}, B, sr, seconds, fmt, d_audio, nullptr, 0, nullptr);
     if (rc) return rc;
     TS_CUDA(cudaMemcpyAsync(host_audio, d_audio, abytes, cudaMemcpyDeviceToHost, S.cur->stream));
     if (host_params)
         TS_CUDA(cudaMemcpyAsync(host_params, d_params, (size_t)B * sizeof(ts_voice), cudaMemcpyDeviceToHost, S.cur->stream));
-    TS_CUDA(cudaStreamSynchronize(S.cur->stream));
-    return TS_OK;
+    return ts_sync();
 }
 
-int ts_corpus_render(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds,
-                     ts_voice *d_params_ring, float *d_audio_ring, int n_ring) {
+int ts_render_host(uint64_t seed, uint64_t batch_index, int B, int sr, double seconds, float *host_audio,
+                   ts_voice *host_params) {
+    return ts_render_host_fmt(seed, batch_index, B, sr, seconds, TS_F32, host_audio, host_params);
+}
+
+int ts_corpus_render_fmt(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds, int fmt,
+                         ts_voice *d_params_ring, void *d_audio_ring, int n_ring) {
     if (!d_params_ring || !d_audio_ring) return fail(TS_ENULL, "NULL ring%s");
     if (n_batches <= 0 || n_ring <= 0) return fail(TS_EINVAL, "n_batches and n_ring must be positive%s");
+    if (S.corpus.open) return fail(TS_EINVAL, "a corpus iterator is open: close it first%s");
     int64_t N;
     int K;
     int rc = check_sizes(B, sr, seconds, &N, &K);
     if (rc) return rc;
+    if (!fmt_ok(fmt)) return fail(TS_EINVAL, "unknown output format%s");
     S.cur = &S.lane[0];
     rc = prepare_common(sr);  // nebula / tables go up on the caller's stream, before the fork
     if (rc) return rc;
-    if (!S.fork) {
-        int lo_p = 0, hi_p = 0;
-        TS_CUDA(cudaDeviceGetStreamPriorityRange(&lo_p, &hi_p));  // numerically lower = higher priority
-        TS_CUDA(cudaStreamCreateWithPriority(&S.hi, cudaStreamNonBlocking, hi_p));
-        TS_CUDA(cudaStreamCreateWithPriority(&S.lo, cudaStreamNonBlocking, lo_p));
-        for (int l = 1; l < TS_LANES; ++l) {
-            S.lane[l].stream = S.hi;
-            S.lane[l].audio_stream = S.lo;
-            TS_CUDA(cudaEventCreateWithFlags(&S.lane[l].ctl_done, cudaEventDisableTiming));
-            TS_CUDA(cudaEventCreateWithFlags(&S.lane[l].aud_done, cudaEventDisableTiming));
-        }
-        TS_CUDA(cudaEventCreateWithFlags(&S.fork, cudaEventDisableTiming));
-    }
-    // fork: both internal streams start after everything already queued on the caller's stream
-    TS_CUDA(cudaEventRecord(S.fork, S.lane[0].stream));
-    TS_CUDA(cudaStreamWaitEvent(S.hi, S.fork, 0));
-    TS_CUDA(cudaStreamWaitEvent(S.lo, S.fork, 0));
-    const bool timing = S.timing;
-    S.timing = false;  // per-kernel events would serialise the streams
-    // Ring hazards: records are written by the sampler and read by the control kernel, both on `hi` in batch order;
-    // audio slots are written by the audio kernels, all on `lo` in batch order.  Nothing else to order.
+    rc = ensure_streams();
+    if (rc) return rc;
+    rc = fork_streams();
+    if (rc) return rc;
+    // Ring hazards: records are written by the setup kernel and read by nothing else on the device; audio slots are
+    // written by the audio kernels, all on `lo` in batch order.  Nothing else to order.
+    const size_t es = fmt_bytes(fmt);
+    int64_t launches = 0;
     for (int i = 0; i < n_batches && rc == TS_OK; ++i) {
-        ts_lane &L = S.lane[1 + (i & 1)];
         const size_t slot = (size_t)(i % n_ring);
-        ts_voice *p = d_params_ring + slot * (size_t)B;
-        float *a = d_audio_ring + slot * (size_t)B * (size_t)N;
-        cudaError_t e = ts_launch_sample(seed, (first_batch + (uint64_t)i) * (uint64_t)B, B, p, L.stream);
-        if (e != cudaSuccess) { rc = cuda_fail(e, "ts_launch_sample"); break; }
-        S.cur = &L;
-        rc = render_impl(p, B, sr, seconds, a, nullptr, 0, nullptr);
+        rc = stream_batch(seed, first_batch + (uint64_t)i, B, sr, seconds, fmt, d_params_ring + slot * (size_t)B,
+                          static_cast<char *>(d_audio_ring) + slot * (size_t)B * (size_t)N * es);
+        launches += S.stats[0];
     }
-    S.cur = &S.lane[0];
-    S.timing = timing;
     // join: the caller's stream continues after both internal streams
     TS_CUDA(cudaEventRecord(S.lane[1].ctl_done, S.hi));
     TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.lane[1].ctl_done, 0));
     TS_CUDA(cudaEventRecord(S.lane[2].ctl_done, S.lo));
     TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.lane[2].ctl_done, 0));
-    S.stats[0] *= n_batches;  // kernels launched by this call (3 per batch and voice chunk: sampler counted below)
-    S.stats[0] += n_batches;
+    S.stats[0] = launches;  // kernels launched by this call (3 per batch and voice chunk)
     return rc;
+}
+
+int ts_corpus_render(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds,
+                     ts_voice *d_params_ring, float *d_audio_ring, int n_ring) {
+    return ts_corpus_render_fmt(seed, first_batch, n_batches, B, sr, seconds, TS_F32, d_params_ring, d_audio_ring, n_ring);
+}
+
+int ts_corpus_open(const ts_corpus_cfg *host_cfg, uint64_t first_batch) {
+    if (!host_cfg) return fail(TS_ENULL, "host_cfg is NULL%s");
+    if (!host_cfg->d_audio_ring || !host_cfg->d_params_ring) return fail(TS_ENULL, "NULL ring%s");
+    if (host_cfg->n_ring < 2 || host_cfg->n_ring > TS_MAX_RING) return fail(TS_EINVAL, "n_ring must be in [2, 64]%s");
+    if (S.corpus.open) return fail(TS_EINVAL, "a corpus iterator is already open%s");
+    int64_t N;
+    int K;
+    int rc = check_sizes(host_cfg->B, host_cfg->sr, host_cfg->seconds, &N, &K);
+    if (rc) return rc;
+    if (!fmt_ok(host_cfg->fmt)) return fail(TS_EINVAL, "unknown output format%s");
+    S.cur = &S.lane[0];
+    rc = prepare_common(host_cfg->sr);
+    if (rc) return rc;
+    rc = ensure_streams();
+    if (rc) return rc;
+    ts_corpus_state &C = S.corpus;
+    C.cfg = *host_cfg;
+    C.N = N;
+    C.next_out = C.next_render = first_batch;
+    for (int i = 0; i < host_cfg->n_ring; ++i)
+        if (!C.ready[i]) TS_CUDA(cudaEventCreateWithFlags(&C.ready[i], cudaEventDisableTiming));
+    if (!C.consumed) TS_CUDA(cudaEventCreateWithFlags(&C.consumed, cudaEventDisableTiming));
+    rc = fork_streams();
+    if (rc) return rc;
+    C.open = true;
+    for (int i = 0; i < host_cfg->n_ring - 1; ++i) {  // render ahead: every slot but one
+        rc = corpus_issue(C.next_render++);
+        if (rc) return rc;
+    }
+    return TS_OK;
+}
+
+int ts_corpus_next(ts_corpus_batch *host_out) {
+    if (!host_out) return fail(TS_ENULL, "host_out is NULL%s");
+    ts_corpus_state &C = S.corpus;
+    if (!C.open) return fail(TS_EINVAL, "no corpus iterator is open%s");
+    // The slot handed out by the previous call is free once the caller's stream reaches this point, and it is the one
+    // slot not in flight: the batch n_ring - 1 ahead of the one handed out now goes into it, ordered after the caller's
+    // stream (both internal streams wait for it).
+    TS_CUDA(cudaEventRecord(C.consumed, S.lane[0].stream));
+    TS_CUDA(cudaStreamWaitEvent(S.lo, C.consumed, 0));
+    TS_CUDA(cudaStreamWaitEvent(S.hi, C.consumed, 0));
+    const int rc = corpus_issue(C.next_render++);
+    if (rc) return rc;
+    const uint64_t b = C.next_out++;
+    const int slot = (int)(b % (uint64_t)C.cfg.n_ring);
+    TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, C.ready[slot], 0));  // the caller's stream waits for this batch
+    host_out->d_audio = static_cast<char *>(C.cfg.d_audio_ring) + (size_t)slot * (size_t)C.cfg.B * (size_t)C.N * fmt_bytes(C.cfg.fmt);
+    host_out->d_params = C.cfg.d_params_ring + (size_t)slot * (size_t)C.cfg.B;
+    host_out->batch_index = b;
+    host_out->first_voice = b * (uint64_t)C.cfg.B;
+    host_out->is_test_first = ts_corpus_is_test(host_out->first_voice);
+    host_out->is_test_last = ts_corpus_is_test(host_out->first_voice + (uint64_t)C.cfg.B - 1);
+    host_out->slot = slot;
+    return TS_OK;
+}
+
+int ts_corpus_close(void) {
+    ts_corpus_state &C = S.corpus;
+    if (!C.open) return TS_OK;
+    C.open = false;
+    TS_CUDA(cudaStreamSynchronize(S.hi));
+    TS_CUDA(cudaStreamSynchronize(S.lo));
+    return TS_OK;
 }
 
 int ts_set_stream(void *cuda_stream) {
@@ -390,6 +578,10 @@ int ts_set_nebula(const ts_range *host_in78) {
             const ts_range &r = host_in78[i];
             if (!(r.curve > 0.0) || !isfinite(r.lo) || !isfinite(r.hi) || !isfinite(r.curve))
                 return fail(TS_EINVAL, "nebula entries must be finite with curve > 0%s");
+            // weights (LFO shapes 35..39, 43..47; modulation mixer 48..67) are normalised by their sum: a negative
+            // range would make w / sum(w), and with it the pitch, unbounded
+            const bool weight = (i >= 35 && i <= 39) || (i >= 43 && i <= 47) || (i >= 48 && i <= 67);
+            if (weight && (r.lo < 0.0 || r.hi < 0.0)) return fail(TS_EINVAL, "nebula ranges of weights must not be negative%s");
         }
         memcpy(S.nebula, host_in78, sizeof S.nebula);
     }
@@ -402,23 +594,42 @@ size_t ts_workspace_bytes(int B, int sr, double seconds) {
     int64_t N;
     int K;
     if (check_sizes(B, sr, seconds, &N, &K)) return 0;
-    return ws_layout(chunk_voices(B, K), K, nullptr);
+    return ws_layout(chunk_voices(B, K), K, true).total;
 }
 
 const char *ts_last_error(void) { return S.err; }
 
 int ts_sync(void) {
-    TS_CUDA(cudaStreamSynchronize(S.lane[0].stream));
-    if (S.lane[0].h_active) S.stats[2] = (int64_t)*S.lane[0].h_active;
+    ts_lane &ln = S.lane[0];
+    // the error flags of all lanes (the streaming calls join the set stream before they return)
+    for (int l = 0; l < TS_LANES; ++l)
+        if (S.lane[l].d_err)
+            TS_CUDA(cudaMemcpyAsync(S.lane[l].h_err, S.lane[l].d_err, sizeof(unsigned int), cudaMemcpyDeviceToHost, ln.stream));
+    TS_CUDA(cudaStreamSynchronize(ln.stream));
+    if (ln.h_active) S.stats[2] = (int64_t)*ln.h_active;
+    bool bad = false;
+    for (int l = 0; l < TS_LANES; ++l)
+        if (S.lane[l].h_err && *S.lane[l].h_err) {
+            bad = true;
+            *S.lane[l].h_err = 0;
+            cudaMemsetAsync(S.lane[l].d_err, 0, sizeof(unsigned int), ln.stream);
+        }
+    if (bad) return fail(TS_ECUDA, "a control kernel gave up waiting for a predecessor chunk (look-back timeout)%s");
     return TS_OK;
 }
 
 void ts_shutdown(void) {
+    if (S.corpus.open) ts_corpus_close();
+    for (auto &e : S.corpus.ready)
+        if (e) { cudaEventDestroy(e); e = nullptr; }
+    if (S.corpus.consumed) { cudaEventDestroy(S.corpus.consumed); S.corpus.consumed = nullptr; }
     for (int l = 0; l < TS_LANES; ++l) {
         ts_lane &L = S.lane[l];
         if (L.ws) cudaFree(L.ws);
         if (L.d_active) cudaFree(L.d_active);
         if (L.h_active) cudaFreeHost(L.h_active);
+        if (L.d_err) cudaFree(L.d_err);
+        if (L.h_err) cudaFreeHost(L.h_err);
         if (L.ctl_done) cudaEventDestroy(L.ctl_done);
         if (L.aud_done) cudaEventDestroy(L.aud_done);
         const cudaStream_t keep = (l == 0) ? L.stream : nullptr;
@@ -429,10 +640,13 @@ void ts_shutdown(void) {
     if (S.hi) { cudaStreamDestroy(S.hi); S.hi = nullptr; }
     if (S.lo) { cudaStreamDestroy(S.lo); S.lo = nullptr; }
     if (S.stage) cudaFree(S.stage);
+    if (S.mmd_ws) cudaFree(S.mmd_ws);
     for (auto &e : S.ev)
         if (e) { cudaEventDestroy(e); e = nullptr; }
     S.stage = nullptr;
     S.stage_bytes = 0;
+    S.mmd_ws = nullptr;
+    S.mmd_ws_count = 0;
     S.cur = &S.lane[0];
     S.nebula_dirty = true;
     S.math_uploaded = false;
@@ -449,33 +663,39 @@ int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, flo
     S.cur = &S.lane[0];
     rc = prepare_common(sr);
     if (rc) return rc;
-    const int Bc = chunk_voices(B, K);
-    size_t off_hdr, off_agg;
-    rc = ensure_ws(ws_layout(Bc, K, &off_hdr, &off_agg));
+    rc = prepare_lane();
     if (rc) return rc;
-    ts_tick *table = reinterpret_cast<ts_tick *>(S.cur->ws);
-    ts_vhdr *hdr = reinterpret_cast<ts_vhdr *>(static_cast<char *>(S.cur->ws) + off_hdr);
-    void *agg = static_cast<char *>(S.cur->ws) + off_agg;
+    const int Bc = chunk_voices(B, K);
+    const ws_layout_t L = ws_layout(Bc, K, true);
+    rc = ensure_ws(L, Bc, K);
+    if (rc) return rc;
+    ts_lane &ln = *S.cur;
+    char *ws = static_cast<char *>(ln.ws);
+    ts_tick *table = reinterpret_cast<ts_tick *>(ws);
+    ts_vhdr *hdr = reinterpret_cast<ts_vhdr *>(ws + L.off_hdr);
+    ts_voice_consts *vc = reinterpret_cast<ts_voice_consts *>(ws + L.off_vc);
+    void *agg = ws + L.off_agg;
     for (auto &e : S.ev)
         if (!e) TS_CUDA(cudaEventCreate(&e));
-    cudaStream_t st = S.cur->stream;
+    cudaStream_t st = ln.stream;
+    const int tails = tails_expected(seconds);
     float a = 0.f, b = 0.f;
     for (int b0 = 0; b0 < B; b0 += Bc) {  // voice chunk by voice chunk, as ts_render launches them
         const int nb = (B - b0 < Bc) ? (B - b0) : Bc;
         TS_CUDA(cudaEventRecord(S.ev[0], st));
         for (int r = 0; r < reps; ++r) {
-            if (++S.cur->epoch == 0) {
-                TS_CUDA(cudaMemsetAsync(agg, 0, ts_control_agg_bytes(Bc, K), st));
-                S.cur->epoch = 1;
+            if (++ln.epoch == 0) {
+                TS_CUDA(cudaMemsetAsync(agg, 0, L.agg_bytes, st));
+                ln.epoch = 1;
             }
-            TS_CUDA(ts_launch_control(d_params + b0, nb, sr, N, K, table, hdr, agg, S.cur->epoch, nullptr, nullptr, nullptr, 0,
-                                      st));
+            TS_CUDA(ts_launch_setup(const_cast<ts_voice *>(d_params) + b0, 0, 0, 0, nb, sr, TS_R, N, K, vc, hdr, nullptr, nullptr, 0, st));
+            TS_CUDA(ts_launch_control(vc, nb, sr, TS_R, N, K, table, agg, ln.epoch, nullptr, 1, ln.d_err, st));
         }
         TS_CUDA(cudaEventRecord(S.ev[1], st));
         for (int r = 0; r < reps; ++r)
             TS_CUDA(ts_launch_audio(table, hdr, nb, N, K,
-                                    d_audio_ring + (size_t)(r % n_ring) * (size_t)B * (size_t)N + (size_t)b0 * (size_t)N, 0,
-                                    tails_expected(seconds), nullptr, st));
+                                    d_audio_ring + (size_t)(r % n_ring) * (size_t)B * (size_t)N + (size_t)b0 * (size_t)N, TS_F32,
+                                    0, tails, nullptr, st));
         TS_CUDA(cudaEventRecord(S.ev[2], st));
         TS_CUDA(cudaEventSynchronize(S.ev[2]));
         float x = 0.f, y = 0.f;
@@ -486,6 +706,23 @@ int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, flo
     }
     host_ms[0] = a / (float)reps;
     host_ms[1] = b / (float)reps;
+    return TS_OK;
+}
+
+int ts_time_fill(void *d_dst, size_t bytes, int reps, float *host_ms) {
+    if (!d_dst || !host_ms) return fail(TS_ENULL, "NULL argument%s");
+    if (bytes < 16 || reps <= 0) return fail(TS_EINVAL, "bytes and reps must be positive%s");
+    for (auto &e : S.ev)
+        if (!e) TS_CUDA(cudaEventCreate(&e));
+    cudaStream_t st = S.lane[0].stream;
+    TS_CUDA(ts_launch_fill(d_dst, bytes, st));
+    TS_CUDA(cudaEventRecord(S.ev[0], st));
+    for (int r = 0; r < reps; ++r) TS_CUDA(ts_launch_fill(d_dst, bytes, st));
+    TS_CUDA(cudaEventRecord(S.ev[1], st));
+    TS_CUDA(cudaEventSynchronize(S.ev[1]));
+    float x = 0.f;
+    TS_CUDA(cudaEventElapsedTime(&x, S.ev[0], S.ev[1]));
+    *host_ms = x / (float)reps;
     return TS_OK;
 }
 
@@ -506,6 +743,33 @@ int ts_last_stats(int64_t host_stats[3]) {
     return TS_OK;
 }
 
+int ts_render_controls_r(const ts_voice *d_params, int B, int sr, double seconds, int R, double *d_ctl) {
+    if (!d_params || !d_ctl) return fail(TS_ENULL, "NULL argument%s");
+    if (R <= 0) return fail(TS_EINVAL, "R must be positive%s");
+    return render_impl(const_cast<ts_voice *>(d_params), sample_spec{false, 0, 0}, B, sr, seconds, TS_F32, nullptr, nullptr, 4, d_ctl, R);
+}
+int ts_render_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl) {
+    return ts_render_controls_r(d_params, B, sr, seconds, TS_R, d_ctl);
+}
+
+int ts_mmd_l1(const float *d_x, const float *d_y, int n, int d, double *d_out) {
+    if (!d_x || !d_y || !d_out) return fail(TS_ENULL, "NULL argument%s");
+    if (n <= 0 || d <= 0 || n > 65535) return fail(TS_EINVAL, "n must be in [1, 65535] and d positive%s");
+    const size_t need = ts_mmd_partial_count(n);
+    if (need > S.mmd_ws_count) {
+        if (S.mmd_ws) cudaFree(S.mmd_ws);
+        S.mmd_ws = nullptr;
+        S.mmd_ws_count = 0;
+        if (cudaMalloc(&S.mmd_ws, need * sizeof(double)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(TS_ENOMEM, "MMD workspace allocation failed%s");
+        }
+        S.mmd_ws_count = need;
+    }
+    TS_CUDA(ts_launch_mmd(d_x, d_y, n, d, S.mmd_ws, d_out, S.lane[0].stream));
+    return TS_OK;
+}
+
 int ts_debug_noise_u32(const uint32_t host_key[2], uint64_t n0, int count, uint32_t *d_out) {
     if (!host_key || !d_out) return fail(TS_ENULL, "NULL argument%s");
     if (count <= 0) return fail(TS_EINVAL, "count must be positive%s");
@@ -514,15 +778,12 @@ int ts_debug_noise_u32(const uint32_t host_key[2], uint64_t n0, int count, uint3
 }
 int ts_debug_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl) {
     if (!d_params || !d_ctl) return fail(TS_ENULL, "NULL argument%s");
-    return render_impl(d_params, B, sr, seconds, nullptr, nullptr, 3, d_ctl);
-}
-int ts_render_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl) {
-    return ts_debug_controls(d_params, B, sr, seconds, d_ctl);
+    return render_impl(const_cast<ts_voice *>(d_params), sample_spec{false, 0, 0}, B, sr, seconds, TS_F32, nullptr, nullptr, 3, d_ctl);
 }
 int ts_debug_phase(const ts_voice *d_params, int B, int sr, double seconds, int vco, double *d_phase) {
     if (!d_params || !d_phase) return fail(TS_ENULL, "NULL argument%s");
     if (vco != 1 && vco != 2) return fail(TS_EINVAL, "vco must be 1 or 2%s");
-    return render_impl(d_params, B, sr, seconds, nullptr, nullptr, vco, d_phase);
+    return render_impl(const_cast<ts_voice *>(d_params), sample_spec{false, 0, 0}, B, sr, seconds, TS_F32, nullptr, nullptr, vco, d_phase);
 }
 
 }  // extern "C"

@@ -64,6 +64,15 @@ __device__ __forceinline__ ts_f2 ts_add2(ts_f2 a, ts_f2 b) {
     return d;
 }
 __device__ __forceinline__ ts_f2 ts_dup(float c) { return ts_pack(c, c); }
+// two fp32 samples -> one 32-bit word of two fp16 / bf16 samples (round to nearest even), first sample in the low half
+template <int FMT> __device__ __forceinline__ uint32_t ts_cvt16(ts_f2 v) {
+    float lo, hi;
+    ts_unpack(v, lo, hi);
+    uint32_t d;
+    if (FMT == TS_F16) asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+    else asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+    return d;
+}
 
 // sin(th) for th in [-pi/2, pi/2] as th + th^3 q(th^2), q minimax of degree 3 (fit of (sin x / x - 1) / x^2 with
 // relative weighting): relative accuracy 1.2e-7 in fp32 down to th -> 0, which the square/saw needs (its tanh
@@ -72,13 +81,17 @@ constexpr float SIN_C3 = -0.16666659712791443f, SIN_C5 = 0.008333087898790836f, 
                 SIN_C9 = 2.6089039693033556e-06f;
 // TAIL = 1: the silent tails are written by the audible CTAs (below); TAIL = 0: every silent tile is written by a CTA of
 // its own (better when few tiles are silent: no zero buffer, more L1 left for the control table).
-template <int MODE, int TAIL>
+// FMT: output sample format (TS_F32 / TS_F16 / TS_BF16): the finished fp32 sample is rounded once, two samples per
+// cvt.rn.{f16x2,bf16x2}.f32, on its way into the staging tile.
+template <int MODE, int TAIL, int FMT>
 __global__ void __launch_bounds__(TS_AUDIO_THREADS)
 ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ hdr, int B, long long N, int K,
-                float *__restrict__ audio, double *__restrict__ dbg_phase, int aligned, uint32_t one_bits) {
+                void *__restrict__ audio_, double *__restrict__ dbg_phase, int aligned, uint32_t one_bits) {
     __shared__ __align__(128) float4 stage[TS_TILE / 4];
     __shared__ __align__(128) float4 zero[(MODE == 0 && TAIL) ? TS_TILE / 4 : 4];  // source of the tail's zero-fill bulk copies
 
+    constexpr int ES = (FMT == TS_F32) ? 4 : 2;  // bytes per output sample
+    char *audio = static_cast<char *>(audio_);
     const int voice = blockIdx.x % B;  // time-major grid: the audible (expensive) tiles are dispatched first
     const long long tile = blockIdx.x / B;
     const long long n_tile0 = tile * TS_TILE;
@@ -86,14 +99,16 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
     const ts_vhdr hd = hdr[voice];
     const long long rem = N - n_tile0;
     const int count = (rem < TS_TILE) ? (int)rem : TS_TILE;  // samples of this tile inside the buffer
-    float *row = audio + (size_t)voice * N + n_tile0;
+    char *row = audio + ((size_t)voice * N + n_tile0) * ES;
 
     if (MODE == 0 && !TAIL && n_tile0 >= hd.n_act) {  // silent tile: exact zeros (S4 release over; pin P9)
         if (aligned) {
             float4 *r4 = reinterpret_cast<float4 *>(row);
-            for (int i = tid; i < count / 4; i += TS_AUDIO_THREADS) r4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int i = tid; i < count * ES / 16; i += TS_AUDIO_THREADS) r4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        } else if (FMT == TS_F32) {
+            for (int i = tid; i < count; i += TS_AUDIO_THREADS) reinterpret_cast<float *>(row)[i] = 0.f;
         } else {
-            for (int i = tid; i < count; i += TS_AUDIO_THREADS) row[i] = 0.f;
+            for (int i = tid; i < count; i += TS_AUDIO_THREADS) reinterpret_cast<unsigned short *>(row)[i] = 0;
         }
         return;
     }
@@ -106,7 +121,7 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
         long long A = ((long long)hd.n_act + TS_TILE - 1) / TS_TILE;
         if (A < 1) A = 1;  // a voice with no audible sample: tile 0 renders zeros and owns the whole tail
         if (tile >= A) return;
-        float *vrow = audio + (size_t)voice * N;
+        char *vrow = audio + (size_t)voice * N * ES;
         if (A + tile >= T) {
             // no silent tile falls to this CTA
         } else if (aligned) {
@@ -118,7 +133,7 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
                 const uint32_t zs = (uint32_t)__cvta_generic_to_shared(zero);
                 for (long long tz = A + tile + (tid >> 5) * A; tz < T; tz += (TS_AUDIO_THREADS / 32) * A) {
                     const long long rz = N - tz * TS_TILE;
-                    ts_bulk_issue(vrow + tz * TS_TILE, zs, (rz < TS_TILE) ? (uint32_t)rz * 4u : (uint32_t)TS_TILE * 4u);
+                    ts_bulk_issue(vrow + tz * TS_TILE * ES, zs, ((rz < TS_TILE) ? (uint32_t)rz : (uint32_t)TS_TILE) * ES);
                 }
                 asm volatile("cp.async.bulk.commit_group;" ::: "memory");
             }
@@ -126,14 +141,19 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
             for (long long tz = A + tile; tz < T; tz += A) {
                 const long long rz = N - tz * TS_TILE;
                 const int cz = (rz < TS_TILE) ? (int)rz : TS_TILE;
-                for (int i = tid; i < cz; i += TS_AUDIO_THREADS) vrow[tz * TS_TILE + i] = 0.f;
+                if (FMT == TS_F32)
+                    for (int i = tid; i < cz; i += TS_AUDIO_THREADS) reinterpret_cast<float *>(vrow)[tz * TS_TILE + i] = 0.f;
+                else
+                    for (int i = tid; i < cz; i += TS_AUDIO_THREADS) reinterpret_cast<unsigned short *>(vrow)[tz * TS_TILE + i] = 0;
             }
         }
     }
 
     const long long r = tile * TS_AUDIO_THREADS + tid;  // run index inside the voice
     const long long n0 = r * TS_RUN;
+    // this thread's 20 samples inside the staging tile: 80 bytes (fp32) or 40 bytes (16-bit formats), conflict-free
     float4 *my = &stage[tid * (TS_RUN / 4)];
+    uint2 *my16 = reinterpret_cast<uint2 *>(reinterpret_cast<char *>(stage) + tid * (TS_RUN * 2));
 
     if (n0 < hd.n_act || (MODE != 0 && n0 < N)) {
         const int j = (int)(r / TS_RUNS_PER_TICK);
@@ -219,7 +239,8 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
                     O[h] = ts_fma2(G3, Z, ts_fma2(G2, Y2, ts_mul2(G1, Y1)));
                     G1 = ts_add2(G1, DG1); G2 = ts_add2(G2, DG2); G3 = ts_add2(G3, DG3);
                 }
-                my2[g] = make_ulonglong2(O[0], O[1]);
+                if (FMT == TS_F32) my2[g] = make_ulonglong2(O[0], O[1]);
+                else my16[g] = make_uint2(ts_cvt16<FMT>(O[0]), ts_cvt16<FMT>(O[1]));
             }
         } else {
             for (int i = 0; i < TS_RUN; ++i) {
@@ -232,37 +253,53 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
         }
     } else if (MODE == 0) {
 #pragma unroll
-        for (int g = 0; g < TS_RUN / 4; ++g) my[g] = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int g = 0; g < TS_RUN / 4; ++g) {
+            if (FMT == TS_F32) my[g] = make_float4(0.f, 0.f, 0.f, 0.f);
+            else my16[g] = make_uint2(0u, 0u);
+        }
     }
     if (MODE != 0) return;
 
     if (aligned) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> async proxy
         __syncthreads();
-        if (tid == 0) ts_bulk_store(row, stage, (uint32_t)count * 4u);
+        if (tid == 0) ts_bulk_store(row, stage, (uint32_t)count * ES);
         else if (TAIL && (tid & 31) == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // zero buffer still being read
     } else {
         __syncthreads();
-        const float *sf = reinterpret_cast<const float *>(stage);
-        for (int i = tid; i < count; i += TS_AUDIO_THREADS) row[i] = sf[i];
+        if (FMT == TS_F32) {
+            const float *sf = reinterpret_cast<const float *>(stage);
+            for (int i = tid; i < count; i += TS_AUDIO_THREADS) reinterpret_cast<float *>(row)[i] = sf[i];
+        } else {
+            const unsigned short *sh = reinterpret_cast<const unsigned short *>(stage);
+            for (int i = tid; i < count; i += TS_AUDIO_THREADS) reinterpret_cast<unsigned short *>(row)[i] = sh[i];
+        }
     }
 }
 
 }  // namespace
 
-cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, float *audio,
+cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, void *audio, int fmt,
                             int mode, int tails, double *dbg_phase, cudaStream_t st) {
     const int64_t tiles = (N + TS_TILE - 1) / TS_TILE;
     const int64_t grid = tiles * B;
     if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
-    const int aligned = (N % 4 == 0) && ((reinterpret_cast<uintptr_t>(audio) & 15u) == 0);
-    if (mode == 0 && tails)
-        ts_audio_kernel<0, 1><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u);
-    else if (mode == 0)
-        ts_audio_kernel<0, 0><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u);
-    else if (mode == 1)
-        ts_audio_kernel<1, 0><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, 0, 0x3f800000u);
-    else
-        ts_audio_kernel<2, 0><<<(unsigned)grid, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, 0, 0x3f800000u);
+    // bulk copies and 128-bit stores need 16-byte aligned rows: N a multiple of 4 (fp32) or 8 (16-bit) samples
+    const int per16 = (fmt == TS_F32) ? 4 : 8;
+    const int aligned = (N % per16 == 0) && ((reinterpret_cast<uintptr_t>(audio) & 15u) == 0);
+    const unsigned g = (unsigned)grid;
+#define TS_LAUNCH(MODE, TAIL, FMT) \
+    ts_audio_kernel<MODE, TAIL, FMT><<<g, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u)
+    if (mode == 0) {
+        if (fmt == TS_F32) { if (tails) TS_LAUNCH(0, 1, TS_F32); else TS_LAUNCH(0, 0, TS_F32); }
+        else if (fmt == TS_F16) { if (tails) TS_LAUNCH(0, 1, TS_F16); else TS_LAUNCH(0, 0, TS_F16); }
+        else if (fmt == TS_BF16) { if (tails) TS_LAUNCH(0, 1, TS_BF16); else TS_LAUNCH(0, 0, TS_BF16); }
+        else return cudaErrorInvalidValue;
+    } else if (mode == 1) {
+        TS_LAUNCH(1, 0, TS_F32);
+    } else {
+        TS_LAUNCH(2, 0, TS_F32);
+    }
+#undef TS_LAUNCH
     return cudaGetLastError();
 }

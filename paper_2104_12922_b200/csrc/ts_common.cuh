@@ -37,6 +37,21 @@ struct __align__(16) ts_vhdr {
 };
 static_assert(sizeof(ts_vhdr) == 32, "ts_vhdr layout");
 
+// ---- per-voice constants: written once per voice by the setup kernel, staged in shared memory by every live
+// chunk CTA of the control kernel -------------------------------------------------------------------------
+struct __align__(16) ts_voice_consts {
+    double h[TS_NPARAM + 2];  // mapped parameters (S2 layout)
+    double rs[18], rd[18], rinv[18];  // per ADSR the three ramps (release, attack, decay): start, duration, 1/duration
+    double lfo_w[2][5];       // LFO shape weights / their sum (0 if the sum is 0)
+    double mix_w[5][4];       // modulation-mixer weights / their row sum
+    double dq_f[2], dq_d[2];  // LFO frequency / cr and rate-mod depth / cr (cycles per tick)
+    double g[3];              // VCA gains: mixer level / level sum; VCO2 also carries (1 - s/2) of S11
+    int jsil;                 // first tick at which the voice is silent for good (== K if never)
+    int slow;                 // some ADSR alpha <= 0: use the generic power
+    int pad[2];
+};
+static_assert(sizeof(ts_voice_consts) % 16 == 0, "ts_voice_consts is copied in 16-byte pieces");
+
 // ---- S0 Philox4x32-10 ---------------------------------------------------------------------------
 __device__ __forceinline__ void ts_philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
                                                  uint32_t k0, uint32_t k1, uint32_t out[4]) {
@@ -64,11 +79,22 @@ cudaError_t ts_launch_noise_debug(uint32_t k0, uint32_t k1, uint64_t n0, int cou
 cudaError_t ts_upload_nebula(const ts_range *host78, cudaStream_t st);
 cudaError_t ts_upload_math_tables(cudaStream_t st);
 size_t ts_control_agg_bytes(int B, int K);  // look-back slots; must be zero before the first launch
+cudaError_t ts_launch_fill(void *d_dst, size_t bytes, cudaStream_t st);  // store-only fill kernel (measurement aid)
+cudaError_t ts_launch_mmd(const float *d_x, const float *d_y, int n, int d, double *d_partial, double *d_out, cudaStream_t st);
+size_t ts_mmd_partial_count(int n);
 // epoch: a value never used before on this `agg` buffer (flags from older launches then read as "not ready")
-cudaError_t ts_launch_control(const ts_voice *d_params, int B, int sr, int64_t N, int K, ts_tick *table,
-                              ts_vhdr *hdr, void *agg, unsigned int epoch, float *params_human, double *dbg_ctl,
-                              unsigned long long *d_active, int full, cudaStream_t st);
+// Per-voice setup (S1 optional, S2/S3, derived constants, last audible tick, header).  sample != 0: draw the records
+// first (S1, global voices g0 .. g0 + B - 1 under `seed`) and write them to d_params; else read d_params.
+// R: samples per control tick (TS_R on the audio path; any R >= 1 for control-rate rendering on its own)
+cudaError_t ts_launch_setup(ts_voice *d_params, int sample, uint64_t seed, uint64_t g0, int B, int sr, int R, int64_t N, int K,
+                            ts_voice_consts *vc, ts_vhdr *hdr, float *params_human, unsigned long long *d_active, int full,
+                            cudaStream_t st);
+// phases != 0: also the S9 tick-level phase scan and the control table (needed by the audio kernel); phases == 0 stops
+// after the modulation mixer (control-rate rendering on its own).  d_err: device flag raised if a look-back wait gives up
+cudaError_t ts_launch_control(const ts_voice_consts *vc, int B, int sr, int R, int64_t N, int K, ts_tick *table, void *agg,
+                              unsigned int epoch, double *dbg_ctl, int phases, unsigned int *d_err, cudaStream_t st);
 // mode 0: audio; mode 1 / 2: write the phase of VCO 1 / 2 (fp64 cycles) to dbg_phase instead.
 // tails != 0: long silent tails are expected (nebula + buffer length), let the audible CTAs write them asynchronously
-cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, float *audio,
+// fmt: TS_F32 / TS_F16 / TS_BF16 output samples
+cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, void *audio, int fmt,
                             int mode, int tails, double *dbg_phase, cudaStream_t st);

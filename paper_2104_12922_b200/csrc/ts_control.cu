@@ -76,18 +76,6 @@ __device__ __forceinline__ double ts_map(double u, const ts_range_dev &r, const 
 }
 
 
-// ---- per-voice constants staged in shared memory by every CTA of the voice ---------------------------
-struct ts_voice_consts {
-    double h[TS_NPARAM + 2];  // mapped parameters (S2 layout)
-    double rs[18], rd[18], rinv[18];  // per ADSR the three ramps (release, attack, decay): start, duration, 1/duration
-    double lfo_w[2][5];       // LFO shape weights / their sum (0 if the sum is 0)
-    double mix_w[5][4];       // modulation-mixer weights / their row sum
-    double dq_f[2], dq_d[2];  // LFO frequency / cr and rate-mod depth / cr (cycles per tick)
-    double g[3];              // VCA gains: mixer level / level sum; VCO2 also carries (1 - s/2) of S11
-    int jsil;                 // first tick at which the voice is silent for good (== K if never)
-    int slow;                 // some ADSR alpha <= 0: use the generic power
-};
-
 // S4 ramp(t,s,d)^alpha.  pow(0,a) = 0 and pow(1,a) = 1 exactly for a > 0, so the saturated ends skip pow.
 // The saturation tests are the oracle's own comparisons (exact); inside the ramp x/d is x * (1/d).
 __device__ __forceinline__ double ts_ramp_pow(double t, double s, double d, double invd, double alpha,
@@ -188,10 +176,22 @@ __device__ __forceinline__ void ts_publish(ts_agg *slot, unsigned long long a, u
     *reinterpret_cast<volatile unsigned int *>(&slot->flag) = epoch;
 }
 // Threads 0..c-1 each fetch one predecessor's aggregate; the sums are combined through shared memory.
-__device__ __forceinline__ void ts_lookback(const ts_agg *slots, int c, unsigned int epoch, unsigned long long *acc /*smem[2]*/) {
+// A predecessor always has a lower block index, so it has been dispatched before this CTA (in-order dispatch of a 1-D
+// grid); the wait is nevertheless bounded: after TS_SPIN_LIMIT polls (about a second) the CTA raises the launch's error
+// flag and goes on with what it has, and the host turns the flag into TS_ECUDA at the next ts_sync().
+constexpr int TS_SPIN_LIMIT = 1 << 24;
+__device__ __forceinline__ void ts_lookback(const ts_agg *slots, int c, unsigned int epoch, unsigned long long *acc /*smem[2]*/,
+                                            unsigned int *err) {
     for (int i = threadIdx.x; i < c; i += blockDim.x) {
         const ts_agg *p = slots + i;
-        while (*reinterpret_cast<const volatile unsigned int *>(&p->flag) != epoch) __nanosleep(20);
+        int spins = 0;
+        while (*reinterpret_cast<const volatile unsigned int *>(&p->flag) != epoch) {
+            __nanosleep(40);
+            if (++spins > TS_SPIN_LIMIT) {
+                atomicExch(err, 1u);
+                break;
+            }
+        }
         __threadfence();
         const unsigned long long a = *reinterpret_cast<const volatile unsigned long long *>(&p->s[0]);
         const unsigned long long b = *reinterpret_cast<const volatile unsigned long long *>(&p->s[1]);
@@ -233,58 +233,52 @@ __device__ __forceinline__ double ts_lfo_mix(double p, const double *wn) {
 constexpr int TS_CTL_THREADS = 128;
 constexpr int TS_CTL_IC = TS_CTL_THREADS - 1;  // control intervals per chunk (the last thread is the halo tick)
 
+// ---- per-voice setup: one CTA per voice ----------------------------------------------------------------------------
+// S1 (optional: the fused sampler of the streaming path), S2/S3 parameter map, the constants every tick needs, the
+// first tick at which the voice is silent for good, and the voice header of the audio kernel.  Everything here used to
+// be recomputed by every chunk CTA of the control kernel (2.3 us each); now it runs once per voice.
 __global__ void __launch_bounds__(TS_CTL_THREADS)
-ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long N, int K, int NC,
-                  ts_tick *__restrict__ table, ts_vhdr *__restrict__ hdr, ts_agg *__restrict__ agg,
-                  unsigned int epoch, float *__restrict__ params_human, double *__restrict__ dbg_ctl,
-                  unsigned long long *__restrict__ d_active, int full) {
+ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64_t g0, int B, int sr, int R, long long N, int K,
+                ts_voice_consts *__restrict__ vc, ts_vhdr *__restrict__ hdr, float *__restrict__ params_human,
+                unsigned long long *__restrict__ d_active, int full) {
     __shared__ ts_voice_consts V;
-    __shared__ ts_math_tables MT;
-    __shared__ unsigned long long scan_sm[64];
-    __shared__ unsigned long long acc[4];
-    __shared__ int s_dead;
-    __shared__ double2 pitch[TS_CTL_THREADS];
-    __shared__ double Es[6][TS_CTL_THREADS];
-
-    const int tid = threadIdx.x;
-    const int c = blockIdx.x / B, v = blockIdx.x - c * B;  // chunk-major: predecessors have lower block indices
-    const ts_voice &rec = params[v];
-    ts_tick *tab = table + (size_t)v * K;
-    ts_agg *agg_q = agg + ((size_t)v * NC) * 2, *agg_p = agg_q + NC;
-
-    // ---- stage tables, map the parameters (S2/S3), derive the per-voice constants ----
-    if (tid < (int)(sizeof(ts_math_tables) / 8))
-        reinterpret_cast<double *>(&MT)[tid] = reinterpret_cast<const double *>(&c_math)[tid];
-    if (tid < 4) acc[tid] = 0ull;
-    if (c > 0 && tid >= 96 && !full) {
-        // Is this whole chunk past the voice's last audible tick?  Only the duration and the four audible releases
-        // decide that: the last warp maps those five parameters straight from the global tables while the others
-        // stage, and evaluates S4's own predicate at the chunk's first tick.  Dead chunks (55 % of C2's) leave now.
-        const int lane = tid - 96;
-        const int idx = (lane == 0) ? 1 : ((lane == 1) ? 5 : ((lane == 2) ? 10 : ((lane == 3) ? 15 : 25)));
-        const double hv = ts_map((double)rec.u[idx], c_nebula[idx], &c_math);
-        const double Dq = __shfl_sync(0xffffffffu, hv, 0);
-        const double r1 = __shfl_sync(0xffffffffu, hv, 1), r2 = __shfl_sync(0xffffffffu, hv, 2);
-        const double r3 = __shfl_sync(0xffffffffu, hv, 3), r4 = __shfl_sync(0xffffffffu, hv, 4);
-        if (lane == 0) {
-            const long long jj = (long long)c * TS_CTL_IC;
-            s_dead = jj >= K || (((double)(jj * TS_R) / (double)sr) - Dq >= fmax(fmax(r1, r2), fmax(r3, r4)));
+    __shared__ __align__(16) float su[TS_NPARAM + 2];
+    __shared__ uint32_t s_nk[2];
+    const int tid = threadIdx.x, v = blockIdx.x;
+    if (sample) {  // S1: Philox blocks 0..19 carry the parameters, thread 20 draws the noise key (D4)
+        const uint64_t g = g0 + (uint64_t)v;
+        const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+        if (tid < 20) {
+            uint32_t w[4];
+            ts_philox4x32_10((uint32_t)tid, (uint32_t)g, (uint32_t)(g >> 32), 0u, k0, k1, w);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) su[4 * tid + i] = (float)(w[i] >> 8) * (1.0f / 16777216.0f);
+        } else if (tid == 20) {
+            uint32_t nk[4];
+            ts_philox4x32_10(0u, (uint32_t)g, (uint32_t)(g >> 32), 2u, k0, k1, nk);
+            s_nk[0] = nk[0];
+            s_nk[1] = nk[1];
         }
-    } else if (tid == 96) {
-        s_dead = 0;
+        __syncthreads();
+        if (tid < 20) {  // the record: u[78] then the two key words, 16 bytes per thread
+            float4 r = *reinterpret_cast<const float4 *>(&su[4 * tid]);
+            if (tid == 19) { r.z = __uint_as_float(s_nk[0]); r.w = __uint_as_float(s_nk[1]); }
+            reinterpret_cast<float4 *>(params + v)[tid] = r;
+        }
+    } else {
+        if (tid < TS_NPARAM) su[tid] = params[v].u[tid];
+        if (tid < 2) s_nk[tid] = params[v].noise_key[tid];
+        __syncthreads();
     }
-    __syncthreads();
-    if (s_dead) return;
     if (tid < TS_NPARAM) {
-        const double hv = ts_map((double)rec.u[tid], c_nebula[tid], &MT);
+        const double hv = ts_map((double)su[tid], c_nebula[tid], &c_math);
         V.h[tid] = hv;
-        if (params_human && c == 0) params_human[(size_t)v * TS_NPARAM + tid] = (float)hv;
+        if (params_human) params_human[(size_t)v * TS_NPARAM + tid] = (float)hv;
     }
     __syncthreads();
     const double *h = V.h;
     const double D = h[1];
-    const double cr = (double)sr / (double)TS_R;
-    const long long J = (N + TS_R - 1) / TS_R;  // control intervals that hold samples
+    const double cr = (double)sr / (double)R;  // control rate (D2): one tick every R samples
     if (tid < 18) {  // ramps of ADSR e: release (starts at D), attack (0), decay (A)
         const int e = tid / 3, k = tid - 3 * e;
         const double A = h[2 + 5 * e], Dc = h[3 + 5 * e], Rl = h[5 + 5 * e];
@@ -321,7 +315,7 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
         long long je = (long long)floor((D + rl_max) * cr) - 8;
         if (je > K) je = K;
         if (je < 0) je = 0;
-        auto silent_at = [&](long long jj) { return jj >= K || (((double)(jj * TS_R) / (double)sr) - D >= rl_max); };
+        auto silent_at = [&](long long jj) { return jj >= K || (((double)(jj * R) / (double)sr) - D >= rl_max); };
         const unsigned int hit = __ballot_sync(0xffffffffu, silent_at(je + lane));
         long long j = hit ? je + (__ffs(hit) - 1) : je + 32;
         if (lane == 0 && (hit & 1u)) {  // estimate off (cannot happen for finite parameters): walk
@@ -331,41 +325,82 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
         }
         j = __shfl_sync(0xffffffffu, j, 0);
         if (tid == 96) {  // one thread writes the results
-        if (full) j = K;  // debug exports: evaluate every tick
-        V.jsil = (int)j;
-        {
+            if (full) j = K;  // debug exports: evaluate every tick
+            V.jsil = (int)j;
             int slow = 0;
             for (int e = 0; e < 6; ++e) slow |= !(h[6 + 5 * e] > 0.0);
             V.slow = slow;
-        }
-        if (c == 0) {
-            const long long n_act = (j * TS_R < N) ? j * TS_R : N;
+            V.pad[0] = V.pad[1] = 0;
+            const long long n_act = (j * R < N) ? j * R : N;
             ts_vhdr hd;
             hd.shape = (float)h[74];
-            const double fc = 440.0 * ts_exp2((h[0] + h[71] - 69.0) * (1.0 / 12.0), &MT);
-            const double k = 12000.0 / (fc * (ts_log2(fc, &MT) * 0.30102999566398120));
+            const double fc = 440.0 * ts_exp2((h[0] + h[71] - 69.0) * (1.0 / 12.0), &c_math);
+            const double k = 12000.0 / (fc * (ts_log2(fc, &c_math) * 0.30102999566398120));
             hd.tanh_c = (float)(1.5707963267948966 * k * 2.0 * 1.4426950408889634);
-            hd.nk0 = rec.noise_key[0];
-            hd.nk1 = rec.noise_key[1];
+            hd.nk0 = s_nk[0];
+            hd.nk1 = s_nk[1];
             hd.n_act = (int32_t)n_act;
             hd.n_ticks = (int32_t)((j + 1 < K) ? j + 1 : K);
             hd.pad[0] = hd.pad[1] = 0;
             hdr[v] = hd;
             if (d_active) atomicAdd(d_active, (unsigned long long)n_act);
         }
-        }
     }
     __syncthreads();
-    const int jsil = V.jsil;
+    if (tid < (int)(sizeof(ts_voice_consts) / 16))
+        reinterpret_cast<uint4 *>(vc + v)[tid] = reinterpret_cast<const uint4 *>(&V)[tid];
+}
+
+// PHASES = 1: controls + the S9 tick-level phase scan + the control table of the audio kernel;
+// PHASES = 0: stops after the modulation mixer (control-rate rendering on its own: no interval sums, no second scan)
+template <int PHASES>
+__global__ void __launch_bounds__(TS_CTL_THREADS)
+ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, long long N, int K, int NC,
+                  ts_tick *__restrict__ table, ts_agg *__restrict__ agg, unsigned int epoch, double *__restrict__ dbg_ctl,
+                  unsigned int *__restrict__ err) {
+    __shared__ ts_voice_consts V;
+    __shared__ ts_math_tables MT;
+    __shared__ unsigned long long scan_sm[64];
+    __shared__ unsigned long long acc[4];
+    __shared__ double2 pitch[TS_CTL_THREADS];
+    __shared__ double Es[6][TS_CTL_THREADS];
+
+    const int tid = threadIdx.x;
+    const int c = blockIdx.x / B, v = blockIdx.x - c * B;  // chunk-major: predecessors have lower block indices
     const int j0 = c * TS_CTL_IC;
-    if (c > 0 && j0 >= jsil) return;  // nothing audible from this chunk on; no successor waits for it
+    const int jsil = vc[v].jsil;
+    if (c > 0 && j0 >= jsil) {  // nothing audible from this chunk on (55 % of C2's chunks); no successor waits for it
+        if (dbg_ctl) {            // control-rate rendering: ticks after the voice has gone silent are 0
+            // ticks j0 + 1 .. j0 + 126, plus the first tick if the previous chunk is dead too (a live one writes its halo)
+            const int j = j0 + tid;
+            const bool prev_live = (c == 1) || (j0 - TS_CTL_IC < jsil);
+            if (tid < TS_CTL_IC && (tid > 0 || !prev_live) && j < K) {
+                double *o = dbg_ctl + (size_t)v * 5 * K;
+#pragma unroll
+                for (int d = 0; d < 5; ++d) o[(size_t)d * K + j] = 0.0;
+            }
+        }
+        return;
+    }
+    ts_tick *tab = table + (size_t)v * K;
+    ts_agg *agg_q = agg + ((size_t)v * NC) * 2, *agg_p = agg_q + NC;
+
+    // ---- stage the math tables and the voice's constants ----
+    if (tid < (int)(sizeof(ts_math_tables) / 8))
+        reinterpret_cast<double *>(&MT)[tid] = reinterpret_cast<const double *>(&c_math)[tid];
+    if (tid < (int)(sizeof(ts_voice_consts) / 16))
+        reinterpret_cast<uint4 *>(&V)[tid] = __ldg(reinterpret_cast<const uint4 *>(vc + v) + tid);
+    if (tid < 4) acc[tid] = 0ull;
+    __syncthreads();
+    const double *h = V.h;
+    const long long J = (N + R - 1) / R;  // control intervals that hold samples (PHASES = 1: R == TS_R)
 
     // ================= phase 1: controls at tick j =================
     const int j = j0 + tid;
     const bool live = (j <= jsil) && (j < K);
     double E[6] = {0, 0, 0, 0, 0, 0};
     unsigned long long dq1 = 0, dq2 = 0;
-    const double tau = (double)((long long)j * TS_R) / (double)sr;
+    const double tau = (double)((long long)j * R) / (double)sr;
     if (V.slow) {  // some alpha <= 0 (custom nebula): generic path, uniform over the voice
         if (live) {
 #pragma unroll 1
@@ -385,32 +420,36 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
     }
     ts_block_scan2(dq1, dq2, scan_sm);  // exclusive prefix inside the chunk
     if (tid == TS_CTL_IC) ts_publish(&agg_q[c], dq1, dq2, epoch);  // halo thread: sum over the chunk's own 127 ticks
-    ts_lookback(agg_q, c, epoch, &acc[0]);
+    ts_lookback(agg_q, c, epoch, &acc[0], err);
     __syncthreads();
     const unsigned long long q1 = ts_frac_q64(h[34]) + acc[0] + dq1, q2 = ts_frac_q64(h[42]) + acc[1] + dq2;
+    // the halo tick is written by the next chunk unless that chunk has nothing to do
+    const bool own = (tid < TS_CTL_IC) || (j0 + TS_CTL_IC >= jsil) || (c == NC - 1);
+    double M[5] = {0, 0, 0, 0, 0};
     if (live) {
         const double L1 = E[2] * ts_lfo_mix(ts_q64_to_double(q1), V.lfo_w[0]);
         const double L2 = E[4] * ts_lfo_mix(ts_q64_to_double(q2), V.lfo_w[1]);
-        double M[5];
 #pragma unroll
         for (int d = 0; d < 5; ++d)
             M[d] = fma(V.mix_w[d][3], L2, fma(V.mix_w[d][2], L1, fma(V.mix_w[d][1], E[1], V.mix_w[d][0] * E[0])));
-        pitch[tid] = make_double2(fma(h[69], M[0], h[0] + h[68]), fma(h[72], M[2], h[0] + h[71]));
-        // the halo tick is written by the next chunk unless that chunk has nothing to do
-        if (tid < TS_CTL_IC || j0 + TS_CTL_IC >= jsil) {
-            float4 a;
-            a.x = (float)(M[1] * V.g[0]);
-            a.y = (float)(M[3] * V.g[1]);
-            a.z = (float)(M[4] * V.g[2]);
-            a.w = 0.0f;
-            *reinterpret_cast<float4 *>(&tab[j].a1) = a;
-            if (dbg_ctl) {
-                double *o = dbg_ctl + (size_t)v * 5 * K;
-#pragma unroll
-                for (int d = 0; d < 5; ++d) o[(size_t)d * K + j] = M[d];
+        if (PHASES) {
+            pitch[tid] = make_double2(fma(h[69], M[0], h[0] + h[68]), fma(h[72], M[2], h[0] + h[71]));
+            if (own) {
+                float4 a;
+                a.x = (float)(M[1] * V.g[0]);
+                a.y = (float)(M[3] * V.g[1]);
+                a.z = (float)(M[4] * V.g[2]);
+                a.w = 0.0f;
+                *reinterpret_cast<float4 *>(&tab[j].a1) = a;
             }
         }
     }
+    if (dbg_ctl && own && j < K) {  // ticks after the voice has gone silent for good are 0
+        double *o = dbg_ctl + (size_t)v * 5 * K;
+#pragma unroll
+        for (int d = 0; d < 5; ++d) o[(size_t)d * K + j] = M[d];
+    }
+    if (!PHASES) return;
     __syncthreads();
 
     // ================= phase 2: interval j (pitch is linear between ticks j and j+1) =================
@@ -442,7 +481,7 @@ ts_control_kernel(const ts_voice *__restrict__ params, int B, int sr, long long 
     }
     ts_block_scan2(s1, s2, scan_sm);
     if (tid == TS_CTL_IC) ts_publish(&agg_p[c], s1, s2, epoch);
-    ts_lookback(agg_p, c, epoch, &acc[2]);
+    ts_lookback(agg_p, c, epoch, &acc[2], err);
     __syncthreads();
     if (act) {
         const unsigned long long P1 = ts_frac_q64(h[70]) + acc[2] + s1, P2 = ts_frac_q64(h[73]) + acc[3] + s2;
@@ -459,16 +498,27 @@ size_t ts_control_agg_bytes(int B, int K) {
     return (size_t)B * NC * 2 * sizeof(ts_agg);
 }
 
-cudaError_t ts_launch_control(const ts_voice *d_params, int B, int sr, int64_t N, int K, ts_tick *table,
-                              ts_vhdr *hdr, void *agg, unsigned int epoch, float *params_human, double *dbg_ctl,
-                              unsigned long long *d_active, int full, cudaStream_t st) {
+cudaError_t ts_launch_setup(ts_voice *d_params, int sample, uint64_t seed, uint64_t g0, int B, int sr, int R, int64_t N, int K,
+                            ts_voice_consts *vc, ts_vhdr *hdr, float *params_human, unsigned long long *d_active, int full,
+                            cudaStream_t st) {
+    ts_setup_kernel<<<(unsigned)B, TS_CTL_THREADS, 0, st>>>(d_params, sample, seed, g0, B, sr, R, (long long)N, K, vc, hdr,
+                                                          params_human, d_active, full);
+    return cudaGetLastError();
+}
+
+cudaError_t ts_launch_control(const ts_voice_consts *vc, int B, int sr, int R, int64_t N, int K, ts_tick *table, void *agg,
+                              unsigned int epoch, double *dbg_ctl, int phases, unsigned int *d_err, cudaStream_t st) {
     const int J = K - 1;
     int NC = (J + TS_CTL_IC - 1) / TS_CTL_IC;
     if (NC < 1) NC = 1;
     const long long grid = (long long)NC * B;
     if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
-    ts_control_kernel<<<(unsigned)grid, TS_CTL_THREADS, 0, st>>>(d_params, B, sr, (long long)N, K, NC, table, hdr,
-                                                                static_cast<ts_agg *>(agg), epoch, params_human,
-                                                                dbg_ctl, d_active, full);
+    if (phases && R != TS_R) return cudaErrorInvalidValue;  // the audio kernel's geometry is built on R = 100
+    if (phases)
+        ts_control_kernel<1><<<(unsigned)grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
+                                                                       static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err);
+    else
+        ts_control_kernel<0><<<(unsigned)grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
+                                                                       static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err);
     return cudaGetLastError();
 }

@@ -1,0 +1,124 @@
+// ts_mmd.cu -- maximum mean discrepancy with the l1 core distance (Eq. 2 at P:L230; reading D25):
+//     MMD(X, Y) = (1/n^2) sum_{i,j} [ 2 |x_i - y_j|_1 - |x_i - x_j|_1 - |y_i - y_j|_1 ]
+// over two sets of n embeddings of dimension d (the paper: n = 1000 sounds, d = 512 OpenL3 values).
+// An l1 distance is not a contraction (no product to accumulate), so there is nothing here for the tensor cores:
+// the work is 2 FADD-class instructions per (pair, component) -- a subtraction and an accumulation of its absolute
+// value -- on the fp32 pipes.  Bound: 2 n_pairs d thread instructions against 148 SMs x 128 lanes per clock; the 4 MB
+// of embeddings stay in L2 and are re-used from shared memory (64 x 64 pairs per CTA, 4 x 4 per thread).
+// The three pair matrices are tiled in one grid; X-X and Y-Y are symmetric, so only tiles on or above the diagonal
+// are computed and the off-diagonal ones count twice.  Per-pair sums are fp32, sums over pairs fp64 in a fixed order
+// (per-CTA partials, then one CTA adds them): bitwise reproducible.
+#include "ts_common.cuh"
+
+namespace {
+
+constexpr int MT = 64;   // pairs per tile side
+constexpr int MK = 32;   // components per shared-memory chunk
+constexpr int MTHREADS = 256;
+
+// tile list: [0, T*T) X-Y tiles (ti, tj); then T(T+1)/2 X-X tiles with tj >= ti; then as many Y-Y tiles
+__device__ __forceinline__ void ts_mmd_tile(int t, int T, int &m, int &ti, int &tj) {
+    const int tri = T * (T + 1) / 2;
+    if (t < T * T) { m = 0; ti = t / T; tj = t - ti * T; return; }
+    t -= T * T;
+    m = 1;
+    if (t >= tri) { t -= tri; m = 2; }
+    int r = 0;  // row r holds T - r tiles
+    while (t >= T - r) { t -= T - r; ++r; }
+    ti = r;
+    tj = r + t;
+}
+
+__global__ void __launch_bounds__(MTHREADS)
+ts_mmd_tiles_kernel(const float *__restrict__ X, const float *__restrict__ Y, int n, int d, int T, double *__restrict__ partial) {
+    __shared__ __align__(16) float As[MK][MT];  // component-major: a thread's four rows are one 128-bit load
+    __shared__ __align__(16) float Bs[MK][MT];
+    __shared__ double red[MTHREADS / 32];
+    int m, ti, tj;
+    ts_mmd_tile((int)blockIdx.x, T, m, ti, tj);
+    const float *A = (m == 2) ? Y : X;
+    const float *Bm = (m == 1) ? X : Y;
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    const int i0 = ti * MT, j0 = tj * MT;
+    float acc[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) acc[a][b] = 0.f;
+
+    for (int k0 = 0; k0 < d; k0 += MK) {
+        // 64 rows x 32 components of each operand; a thread loads component (tid % 32) of rows tid / 32 + 8 p
+#pragma unroll
+        for (int p = 0; p < MT / 8; ++p) {
+            const int r = (tid >> 5) + 8 * p, k = k0 + (tid & 31);
+            As[tid & 31][r] = (i0 + r < n && k < d) ? __ldg(A + (size_t)(i0 + r) * d + k) : 0.f;
+            Bs[tid & 31][r] = (j0 + r < n && k < d) ? __ldg(Bm + (size_t)(j0 + r) * d + k) : 0.f;
+        }
+        __syncthreads();
+#pragma unroll 8
+        for (int kk = 0; kk < MK; ++kk) {
+            const float4 a = *reinterpret_cast<const float4 *>(&As[kk][ty * 4]);
+            const float4 b = *reinterpret_cast<const float4 *>(&Bs[kk][tx * 4]);
+            const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+            for (int p = 0; p < 4; ++p)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) acc[p][q] += fabsf(av[p] - bv[q]);
+        }
+        __syncthreads();
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int p = 0; p < 4; ++p)
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (i0 + ty * 4 + p < n && j0 + tx * 4 + q < n) s += (double)acc[p][q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if ((tid & 31) == 0) red[tid >> 5] = s;
+    __syncthreads();
+    if (tid == 0) {
+        double t = 0.0;
+        for (int w = 0; w < MTHREADS / 32; ++w) t += red[w];
+        partial[blockIdx.x] = (m != 0 && tj > ti) ? 2.0 * t : t;  // the mirrored tile of a symmetric matrix
+    }
+}
+
+__global__ void ts_mmd_final_kernel(const double *__restrict__ partial, int n, int T, double *__restrict__ out) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const int tri = T * (T + 1) / 2;
+    double sxy = 0.0, sxx = 0.0, syy = 0.0;
+    for (int t = 0; t < T * T; ++t) sxy += partial[t];
+    for (int t = 0; t < tri; ++t) sxx += partial[T * T + t];
+    for (int t = 0; t < tri; ++t) syy += partial[T * T + tri + t];
+    out[0] = (2.0 * sxy - sxx - syy) / ((double)n * (double)n);
+    out[1] = sxy;
+    out[2] = sxx;
+    out[3] = syy;
+}
+
+// store-only fill (measurement aid: what a pure 128-bit store stream reaches on this GPU, beside the copy peak)
+__global__ void __launch_bounds__(256) ts_fill_kernel(float4 *__restrict__ dst, size_t n16) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride) dst[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+}  // namespace
+
+size_t ts_mmd_partial_count(int n) {
+    const size_t T = ((size_t)n + MT - 1) / MT;
+    return T * T + T * (T + 1);
+}
+
+cudaError_t ts_launch_mmd(const float *d_x, const float *d_y, int n, int d, double *d_partial, double *d_out, cudaStream_t st) {
+    const int T = (n + MT - 1) / MT;
+    const unsigned tiles = (unsigned)(T * T + T * (T + 1));
+    ts_mmd_tiles_kernel<<<tiles, MTHREADS, 0, st>>>(d_x, d_y, n, d, T, d_partial);
+    ts_mmd_final_kernel<<<1, 32, 0, st>>>(d_partial, n, T, d_out);
+    return cudaGetLastError();
+}
+
+cudaError_t ts_launch_fill(void *d_dst, size_t bytes, cudaStream_t st) {
+    ts_fill_kernel<<<148 * 8, 256, 0, st>>>(static_cast<float4 *>(d_dst), bytes / 16);
+    return cudaGetLastError();
+}
