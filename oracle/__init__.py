@@ -72,6 +72,16 @@ def lib():
         L.orc_render_voice.restype = C.c_int
         L.orc_num_samples.argtypes = [C.c_int, C.c_double]
         L.orc_num_samples.restype = C.c_int64
+        L.orc_num_ticks_r.argtypes = [C.c_int64, C.c_int]
+        L.orc_num_ticks_r.restype = C.c_int64
+        L.orc_controls_r.argtypes = [f64p, C.c_int, C.c_int64, C.c_int, f64p, f64p, f64p]
+        L.orc_upsample_r.argtypes = [f64p, C.c_int64, C.c_int]
+        L.orc_upsample_r.restype = C.c_double
+        L.orc_render_voice_r.argtypes = [f32p, u32p, C.POINTER(Range), C.c_int, C.c_int64, C.c_int, f64p, f64p, f64p, f64p]
+        L.orc_render_voice_r.restype = C.c_int
+        L.orc_mmd_l1.argtypes = [f64p, f64p, C.c_int, C.c_int, f64p]
+        L.orc_mmd_l1.restype = C.c_double
+        L.orc_corpus_is_test.argtypes = [C.c_uint64]
         _lib = L
     return _lib
 
@@ -130,9 +140,63 @@ def adsr(t, A, Dc, S, Rl, alpha, D) -> float:
 
 
 def corpus_is_test(g: int) -> bool:
-    L = lib()
-    L.orc_corpus_is_test.argtypes = [C.c_uint64]
-    return bool(L.orc_corpus_is_test(g))
+    return bool(lib().orc_corpus_is_test(g))
+
+
+def num_ticks_r(N: int, R: int) -> int:
+    return lib().orc_num_ticks_r(N, R)
+
+
+def controls_r(h, sr: int, N: int, R: int):
+    """human params h[78], one control tick every R samples -> (E[6,K], L[2,K], M[5,K]), K = ceil(N/R) + 1."""
+    h = np.ascontiguousarray(h, dtype=np.float64)
+    K = num_ticks_r(N, R)
+    E = np.empty((6, K)); Lf = np.empty((2, K)); M = np.empty((5, K))
+    lib().orc_controls_r(_p(h, C.c_double), sr, N, R, _p(E, C.c_double), _p(Lf, C.c_double), _p(M, C.c_double))
+    return E, Lf, M
+
+
+def upsample_r(Cs, n: int, R: int) -> float:
+    Cs = np.ascontiguousarray(Cs, dtype=np.float64)
+    return lib().orc_upsample_r(_p(Cs, C.c_double), n, R)
+
+
+def render_voice_r(u, noise_key, sr: int, N: int, R: int, neb=None, want_phase: bool = False):
+    """One voice with one control tick every R samples -> dict(audio f64[N], phase1, phase2)."""
+    neb, nptr = _neb_ptr(default_nebula() if neb is None else neb)
+    u = np.ascontiguousarray(u, dtype=np.float32)
+    k = np.ascontiguousarray(noise_key, dtype=np.uint32)
+    audio = np.empty(N, dtype=np.float64)
+    p1 = np.empty(N, dtype=np.float64) if want_phase else None
+    p2 = np.empty(N, dtype=np.float64) if want_phase else None
+    null = C.POINTER(C.c_double)()
+    rc = lib().orc_render_voice_r(_p(u, C.c_float), _p(k, C.c_uint32), nptr, sr, N, R, _p(audio, C.c_double),
+                                  _p(p1, C.c_double) if want_phase else null, _p(p2, C.c_double) if want_phase else null, null)
+    if rc != 0:
+        raise MemoryError("orc_render_voice_r")
+    return {"audio": audio, "phase1": p1, "phase2": p2}
+
+
+def mmd_l1(X, Y):
+    """Eq. 2 with the l1 core distance -> (MMD, [sum d(x,y), sum d(x,x), sum d(y,y)]); X, Y: [n, d]."""
+    X = np.ascontiguousarray(X, dtype=np.float64)
+    Y = np.ascontiguousarray(Y, dtype=np.float64)
+    assert X.shape == Y.shape and X.ndim == 2
+    sums = np.empty(3, dtype=np.float64)
+    v = lib().orc_mmd_l1(_p(X, C.c_double), _p(Y, C.c_double), X.shape[0], X.shape[1], _p(sums, C.c_double))
+    return v, sums
+
+
+def round_bf16(x) -> np.ndarray:
+    """fp64/fp32 values -> the nearest bfloat16 (round to nearest even, through fp32 as the GPU path does), as float32."""
+    b = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32).astype(np.uint64)
+    b = (b + 0x7FFF + ((b >> 16) & 1)) & 0xFFFF0000
+    return b.astype(np.uint32).view(np.float32)
+
+
+def round_f16(x) -> np.ndarray:
+    """fp64/fp32 values -> the nearest IEEE half (round to nearest even, through fp32 as the GPU path does), as float32."""
+    return np.ascontiguousarray(x, dtype=np.float32).astype(np.float16).astype(np.float32)
 
 
 def num_ticks(N: int) -> int:
@@ -199,12 +263,13 @@ def render_voice(u, noise_key, sr: int, N: int, neb=None, want_phase: bool = Fal
     return {"audio": audio, "phase1": p1, "phase2": p2, "human": hm}
 
 
-def render_batch(u, noise_key, sr: int, N: int, neb=None, threads: int | None = None, dtype=np.float64):
+def render_batch(u, noise_key, sr: int, N: int, neb=None, threads: int | None = None, dtype=np.float64, out=None):
     """Voices are independent: render rows on a thread pool (ctypes releases the GIL).
     -> audio [B,N] in `dtype` (float64 = the oracle's own values)."""
     u = np.ascontiguousarray(u, dtype=np.float32)
     B = u.shape[0]
-    out = np.empty((B, N), dtype=dtype)
+    if out is None:
+        out = np.empty((B, N), dtype=dtype)
     threads = threads or os.cpu_count() or 1
 
     def one(b):

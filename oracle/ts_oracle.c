@@ -29,6 +29,11 @@
  *                          cumulative sums on tiny inputs
  *   squaresaw ............ pinned: oddness, limits, zero at theta=pi for s=1, bound 1.125
  *   noise ................ pinned: exact words from the KAT-pinned Philox, moments
+ *   controls_r / upsample_r / render_voice_r (tick spacing R as a parameter):
+ *                          pinned: R = 1 makes upsampling the identity (P7), per-sample ADSR equals orc_adsr(n/sr),
+ *                          LFO closed form at cr = sr, and R = 100 reproduces the fixed-R functions bit for bit
+ *   mmd_l1 ............... pinned: MMD(X,X) = 0 exactly, hand-computed 2x2 case, permutation invariance,
+ *                          translation invariance, linear scaling, an independent library l1 distance matrix
  *   whole-voice audio .... PARITY UNPINNED by the paper (no printed waveform); cross-checked
  *                          against the survey probe values (last row of pins)
  *
@@ -180,8 +185,10 @@ double orc_adsr(double t, double A, double Dc, double S, double Rl, double alpha
     return a * (1.0 - (1.0 - S) * d) * (1.0 - r);
 }
 
-/* number of control ticks, S5: K = ceil(N/R) + 1 */
-int64_t orc_num_ticks(int64_t N) { return (N + ORC_R - 1) / ORC_R + 1; }
+/* number of control ticks, S5: K = ceil(N/R) + 1 (R = ORC_R on the audio path; any R >= 1 for the control-rate
+ * functions with a tick-spacing parameter) */
+int64_t orc_num_ticks_r(int64_t N, int R) { return (N + R - 1) / R + 1; }
+int64_t orc_num_ticks(int64_t N) { return orc_num_ticks_r(N, ORC_R); }
 
 static double orc_frac(double x) { return x - floor(x); }
 
@@ -201,14 +208,14 @@ void orc_lfo_shapes(double p, double sh[5]) {
  * amp-mod ADSR; modulation mixer).
  * Outputs (any may be NULL): E[6][K], L[2][K], M[5][K].
  * ---------------------------------------------------------------------------------------- */
-void orc_controls(const double h[ORC_NPARAM], int sr, int64_t N, double *E_out, double *L_out, double *M_out) {
-    const int64_t K = orc_num_ticks(N);
-    const double cr = (double)sr / (double)ORC_R;
+void orc_controls_r(const double h[ORC_NPARAM], int sr, int64_t N, int R, double *E_out, double *L_out, double *M_out) {
+    const int64_t K = orc_num_ticks_r(N, R);
+    const double cr = (double)sr / (double)R; /* control rate, D2 with R in place of 100 */
     const double D = h[1];
     double q[2] = {h[34], h[42]}; /* q_0 = initial_phase */
     static const int amp_e[2] = {2, 4}, rate_e[2] = {3, 5};
     for (int64_t j = 0; j < K; ++j) {
-        double tau = (double)(j * ORC_R) / (double)sr;
+        double tau = (double)(j * R) / (double)sr;
         double E[6];
         for (int e = 0; e < 6; ++e) {
             const double *a = &h[2 + 5 * e];
@@ -247,11 +254,16 @@ void orc_controls(const double h[ORC_NPARAM], int sr, int64_t N, double *E_out, 
     }
 }
 
-/* S8  Upsample: linear interpolation tick -> sample. */
-double orc_upsample(const double *C, int64_t n) {
-    int64_t j = n / ORC_R, m = n % ORC_R;
-    return C[j] + (C[j + 1] - C[j]) * ((double)m / (double)ORC_R);
+void orc_controls(const double h[ORC_NPARAM], int sr, int64_t N, double *E_out, double *L_out, double *M_out) {
+    orc_controls_r(h, sr, N, ORC_R, E_out, L_out, M_out);
 }
+
+/* S8  Upsample: linear interpolation tick -> sample; tick j sits on sample j*R. */
+double orc_upsample_r(const double *C, int64_t n, int R) {
+    int64_t j = n / R, m = n % R;
+    return C[j] + (C[j + 1] - C[j]) * ((double)m / (double)R);
+}
+double orc_upsample(const double *C, int64_t n) { return orc_upsample_r(C, n, ORC_R); }
 
 /* S11 SquareSaw waveform value at theta (D14). */
 double orc_squaresaw(double theta, double k, double s) {
@@ -278,16 +290,16 @@ double orc_noise_value(uint32_t x) { return (double)(x >> 8) * (1.0 / 8388608.0)
  * S2..S14  Render one voice.  audio[N] (fp64, before the final float rounding); optional
  * phase1[N], phase2[N] (cycles in [0,1)), human[78].  Returns 0, or -1 on allocation failure.
  * ---------------------------------------------------------------------------------------- */
-int orc_render_voice(const float u[ORC_NPARAM], const uint32_t noise_key[2], const orc_range neb[ORC_NPARAM],
-                     int sr, int64_t N, double *audio, double *phase1, double *phase2, double *human) {
+int orc_render_voice_r(const float u[ORC_NPARAM], const uint32_t noise_key[2], const orc_range neb[ORC_NPARAM],
+                       int sr, int64_t N, int R, double *audio, double *phase1, double *phase2, double *human) {
     const double TWO_PI = 6.283185307179586476925286766559;
     double h[ORC_NPARAM];
     orc_map_all(u, neb, h);
     if (human) memcpy(human, h, sizeof h);
-    const int64_t K = orc_num_ticks(N);
+    const int64_t K = orc_num_ticks_r(N, R);
     double *M = (double *)malloc((size_t)(5 * K) * sizeof(double));
     if (!M) return -1;
-    orc_controls(h, sr, N, NULL, NULL, M);
+    orc_controls_r(h, sr, N, R, NULL, NULL, M);
     const double *M_p1 = M + 0 * K, *M_a1 = M + 1 * K, *M_p2 = M + 2 * K, *M_a2 = M + 3 * K, *M_a3 = M + 4 * K;
 
     const double midi = h[0];
@@ -300,7 +312,7 @@ int orc_render_voice(const float u[ORC_NPARAM], const uint32_t noise_key[2], con
 
     for (int64_t n = 0; n < N; ++n) {
         /* S9: exclusive running sum -- sample n uses phi_n */
-        double m1 = orc_upsample(M_p1, n), m2 = orc_upsample(M_p2, n);
+        double m1 = orc_upsample_r(M_p1, n, R), m2 = orc_upsample_r(M_p2, n, R);
         double pitch1 = midi + tune1 + depth1 * m1;
         double pitch2 = midi + tune2 + depth2 * m2;
         double inc1 = (440.0 / (double)sr) * exp2((pitch1 - 69.0) / 12.0);
@@ -313,7 +325,7 @@ int orc_render_voice(const float u[ORC_NPARAM], const uint32_t noise_key[2], con
         /* S12 */
         double z = orc_noise_value(orc_noise_word(noise_key, (uint64_t)n));
         /* S13, S14 */
-        double a1 = orc_upsample(M_a1, n), a2 = orc_upsample(M_a2, n), a3 = orc_upsample(M_a3, n);
+        double a1 = orc_upsample_r(M_a1, n, R), a2 = orc_upsample_r(M_a2, n, R), a3 = orc_upsample_r(M_a3, n, R);
         double out = (lsum == 0.0) ? 0.0 : (l1 * a1 * y1 + l2 * a2 * y2 + l3 * a3 * z) / lsum;
         audio[n] = out;
         phi1 = orc_frac(phi1 + inc1);
@@ -321,6 +333,11 @@ int orc_render_voice(const float u[ORC_NPARAM], const uint32_t noise_key[2], con
     }
     free(M);
     return 0;
+}
+
+int orc_render_voice(const float u[ORC_NPARAM], const uint32_t noise_key[2], const orc_range neb[ORC_NPARAM],
+                     int sr, int64_t N, double *audio, double *phase1, double *phase2, double *human) {
+    return orc_render_voice_r(u, noise_key, neb, sr, N, ORC_R, audio, phase1, phase2, human);
 }
 
 /* D17: N = llround(sr * seconds) */
@@ -331,4 +348,31 @@ int64_t orc_num_samples(int sr, double seconds) { return (int64_t)llround((doubl
 int orc_corpus_is_test(uint64_t g) {
     uint64_t block = g / 1024u;      /* blocks of 1024 consecutive sounds */
     return (block % 10u) == 9u;      /* nine train blocks, then one test block */
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Eq. 2 (Eq. 2 at P:L230): maximum mean discrepancy of two sets X, Y of n elements each with the
+ * l1 distance as the core distance d ("OpenL3 ... l1 as the core distance d"):
+ *     MMD(X, Y) = 1/(n n) * sum_{i,j} [ 2 d(x_i, y_j) - d(x_i, x_j) - d(y_i, y_j) ].
+ * "1/nn" in PAPER.md is garbled; read as 1/n^2 (reading D25), and the sum runs over all n*n ordered pairs
+ * (the printed bounds "i,j=0..n" would count n+1 elements of an n-element set).  X, Y: [n][dim] row-major.
+ * sums (may be NULL): [0] sum d(x_i,y_j), [1] sum d(x_i,x_j), [2] sum d(y_i,y_j).
+ * ---------------------------------------------------------------------------------------- */
+double orc_l1(const double *a, const double *b, int dim) {
+    double s = 0.0;
+    for (int k = 0; k < dim; ++k) s += fabs(a[k] - b[k]);
+    return s;
+}
+
+double orc_mmd_l1(const double *X, const double *Y, int n, int dim, double sums[3]) {
+    double sxy = 0.0, sxx = 0.0, syy = 0.0;
+    for (int i = 0; i < n; ++i) {
+        for (int j = 0; j < n; ++j) {
+            sxy += orc_l1(X + (size_t)i * dim, Y + (size_t)j * dim, dim);
+            sxx += orc_l1(X + (size_t)i * dim, X + (size_t)j * dim, dim);
+            syy += orc_l1(Y + (size_t)i * dim, Y + (size_t)j * dim, dim);
+        }
+    }
+    if (sums) { sums[0] = sxy; sums[1] = sxx; sums[2] = syy; }
+    return (2.0 * sxy - sxx - syy) / ((double)n * (double)n);
 }

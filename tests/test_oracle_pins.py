@@ -553,3 +553,167 @@ def test_corpus_train_test_split_follows_p_l102():
             assert len(flags) == 1
     assert O.corpus_is_test(72 * 128) and O.corpus_is_test(79 * 128 + 127) and not O.corpus_is_test(80 * 128)
     assert O.corpus_is_test(2**40 * 10240 + 9 * 1024 + 5)        # 64-bit indices
+
+
+# ----------------------------------------------------------------------------- VCO2 modulated pitch (S9, row M_2, h[71], h[72])
+def test_s9_vco2_modulated_phase_brute_force_high_precision():
+    """VCO2's phase uses its OWN row (M_2), tuning (h[71]) and depth (h[72]): phi2_n = phi2_0 + sum_{k<n} (440/sr)
+    2^((midi + tune_2 + depth_2 up(M_2)(k) - 69)/12), re-done in 50-digit decimal arithmetic from the oracle's own tick
+    values.  Row M_2 is one-hot on adsr2 while row M_0 (VCO1) listens to adsr1 with another depth and tuning, so a
+    swapped row, tuning or depth index fails; VCO1 is checked in the same render against its own row."""
+    h = neutral_h()
+    h[0], h[70], h[73] = 58.0, 0.2, -0.35
+    h[2:7] = [0.02, 0.01, 0.4, 0.0, 1.7]          # adsr1 moves within the first ticks
+    h[7:12] = [0.005, 0.03, 0.2, 0.0, 0.6]        # adsr2 moves differently
+    h[68], h[69] = 2.0, 17.0                      # vco1 tuning, depth
+    h[71], h[72] = -5.0, -43.0                    # vco2 tuning, depth (negative: pitch falls with the envelope)
+    h[48 + 4 * 0 + 0] = 1.0                       # M_0 <- adsr1
+    h[48 + 4 * 2 + 1] = 1.0                       # M_2 <- adsr2
+    sr, N = 8000, 260
+    E, L, M = O.controls(h, sr, N)
+    assert np.array_equal(M[0], E[0]) and np.array_equal(M[2], E[1]) and not np.array_equal(E[0], E[1])
+    r = render_h(h, N, sr=sr, want_phase=True)
+    decimal.getcontext().prec = 50
+    Dm = decimal.Decimal
+    ln2 = Dm(2).ln()
+    for row, tune, depth, start, key in ((0, 68, 69, 70, "phase1"), (2, 71, 72, 73, "phase2")):
+        phi = Dm(h[start])
+        for n in range(N):
+            d = abs(float(phi % 1) - r[key][n])
+            assert min(d, 1 - d) < 1e-13, (key, n)
+            j, m = divmod(n, 100)
+            ctl = Dm(M[row][j]) + (Dm(M[row][j + 1]) - Dm(M[row][j])) * Dm(m) / Dm(100)
+            pitch = Dm(h[0]) + Dm(h[tune]) + Dm(h[depth]) * ctl
+            phi += Dm(440) / Dm(sr) * ((pitch - 69) / 12 * ln2).exp()
+
+
+def test_s9_vco2_audio_follows_its_modulated_phase():
+    """... and the square/saw is evaluated AT that phase: y2 = orc_squaresaw(2 pi phase2, k(midi, tune_2), s)."""
+    h = neutral_h()
+    h[0], h[71], h[72], h[73], h[74] = 50.0, 7.0, 30.0, 0.1, 0.3
+    h[7:12] = [0.01, 0.02, 0.5, 0.0, 1.3]
+    h[48 + 4 * 2 + 1] = 1.0                       # M_2 <- adsr2
+    h[48 + 4 * 3 + 0] = 1.0; h[76] = 1.0          # vco2 amp <- adsr1 (constant 1), only vco2 in the mix
+    N = 900
+    r = render_h(h, N, want_phase=True)
+    k = O.squaresaw_k(50.0, 7.0)
+    want = np.array([O.squaresaw(2 * np.pi * p, k, 0.3) for p in r["phase2"]])
+    assert np.abs(r["audio"] - want).max() < 1e-9
+    assert np.abs(np.diff(r["phase2"][:200] % 1)).std() > 0          # the pitch really moves
+
+
+# ----------------------------------------------------------------------------- tick spacing R as a parameter (SURVEY 8(f) item 3)
+def test_r100_functions_reproduce_the_fixed_r_ones_bit_for_bit():
+    u, nk = O.sample_params(5, 0, 3)
+    for b in range(3):
+        h = O.map_all(u[b])
+        for a, c in zip(O.controls(h, SR, 4410), O.controls_r(h, SR, 4410, 100)):
+            assert np.array_equal(a, c)
+        assert np.array_equal(O.render_voice(u[b], nk[b], SR, 2000)["audio"], O.render_voice_r(u[b], nk[b], SR, 2000, 100)["audio"])
+    assert O.num_ticks_r(44100, 100) == O.num_ticks(44100) == 442 and O.num_ticks_r(44100, 1) == 44101
+    assert O.num_ticks_r(44101, 7) == 6301 + 1
+
+
+def test_p7_r1_upsampling_is_the_identity():
+    """Pin P7: with one tick per sample (R = 1) the interpolation weight m/R is 0 for every n: up(C)(n) == C[n] exactly."""
+    rng = np.random.default_rng(3)
+    Cs = rng.standard_normal(64)
+    for n in range(63):
+        assert O.upsample_r(Cs, n, 1) == Cs[n]
+    for R in (2, 7, 100):                          # and for any R the tick values are hit and a line is reproduced
+        lin = 0.25 + 0.5 * np.arange(10)
+        for n in range(9 * R):
+            assert O.upsample_r(lin, n, R) == pytest.approx(0.25 + 0.5 * n / R, abs=1e-14)
+            if n % R == 0:
+                assert O.upsample_r(Cs, n, R) == Cs[n // R]
+
+
+def test_r1_controls_are_the_closed_forms_at_every_sample():
+    """R = 1 (audio-rate control): tick j sits on sample j, tau_j = j/sr.  ADSRs equal orc_adsr(j/sr) (itself pinned by
+    P5), and an LFO with no rate modulation has the closed form q_j = q_0 + j f/sr (P6 at cr = sr)."""
+    h = neutral_h(D=0.004)
+    h[2:7] = [0.001, 0.0015, 0.6, 0.002, 2.5]
+    h[32:40] = [250.0, 0.0, 0.125, 1.0, 0.0, 0.0, 0.0, 0.0]     # lfo1: 250 Hz sine, start phase 1/8, no rate modulation
+    h[12:17] = [0.0, 0.0, 1.0, 0.0, 1.0]                        # lfo1_amp == 1 while t < D
+    h[48 + 4 * 1 + 0] = 1.0                                     # M_1 <- adsr1
+    h[48 + 4 * 3 + 2] = 1.0                                     # M_3 <- lfo1
+    sr, N = 8000, 80
+    E, L, M = O.controls_r(h, sr, N, 1)
+    assert E.shape == (6, N + 1)
+    for j in range(N + 1):
+        t = j / sr
+        assert M[1][j] == O.adsr(t, 0.001, 0.0015, 0.6, 0.002, 2.5, 0.004)
+        want = math.sin(2 * math.pi * (0.125 + j * 250.0 / sr)) if t < 0.004 else 0.0
+        assert M[3][j] == pytest.approx(want, abs=1e-12)
+    # the analytic segment values of P5 on the sample grid: E(A) = 1 at j = 8, E(A + Dc) = S at j = 20, 0 after D + Rl
+    assert M[1][8] == pytest.approx(1.0, abs=1e-15) and M[1][20] == pytest.approx(0.6, abs=1e-15)
+    assert np.all(M[1][49:] == 0.0)
+
+
+def test_r1_render_constant_sine_and_r_dependence():
+    """The audio path with R = 1: a constant-frequency sine is still sin(2 pi f t) (P8), and for a moving envelope
+    R = 1 differs from R = 100 exactly as D1 says (the envelope is no longer smeared over 100 samples)."""
+    h = sine_only_h()
+    u = np.full(O.NPARAM, 0.5, dtype=np.float32)
+    nk = np.array([1, 2], dtype=np.uint32)
+    a = O.render_voice_r(u, nk, SR, 3000, 1, fixed_nebula(h))["audio"]
+    assert np.abs(a - np.sin(2 * np.pi * 440 * np.arange(3000) / SR)).max() < 1e-12
+    h[2:7] = [0.003, 0, 1, 0, 1]                                # 132.3-sample linear attack on the amp row
+    a1 = O.render_voice_r(u, nk, SR, 400, 1, fixed_nebula(h))["audio"]
+    a100 = O.render_voice_r(u, nk, SR, 400, 100, fixed_nebula(h))["audio"]
+    n = np.arange(400)
+    s = np.sin(2 * np.pi * 440 * n / SR)
+    assert np.abs(a1 - np.minimum(n / (0.003 * SR), 1.0) * s).max() < 1e-12          # exact envelope per sample
+    e100 = np.interp(n, [0, 100, 200, 300, 400], [0, 100 / 132.3, 1, 1, 1])          # tick values, lerped
+    assert np.abs(a100 - e100 * s).max() < 1e-12
+
+
+# ----------------------------------------------------------------------------- Eq. 2: MMD with the l1 core distance
+def test_mmd_identical_sets_is_exactly_zero():
+    rng = np.random.default_rng(0)
+    X = rng.standard_normal((17, 9))
+    v, sums = O.mmd_l1(X, X)
+    assert v == 0.0 and sums[0] == sums[1] == sums[2]
+
+
+def test_mmd_hand_computed_2x2():
+    """X = {(0,0), (1,2)}, Y = {(3,0), (0,-1)}.  l1 distances: d(x,y) = [[3,1],[4,4]] -> 12; d(x,x) = [[0,3],[3,0]] -> 6;
+    d(y,y) = [[0,4],[4,0]] -> 8.  MMD = (2*12 - 6 - 8) / (2*2) = 2.5   (Eq. 2, 1/n^2 reading)."""
+    v, sums = O.mmd_l1(np.array([[0., 0.], [1., 2.]]), np.array([[3., 0.], [0., -1.]]))
+    assert list(sums) == [12.0, 6.0, 8.0] and v == 2.5
+
+
+def test_mmd_invariances_and_scaling():
+    rng = np.random.default_rng(1)
+    X, Y = rng.standard_normal((23, 11)), rng.standard_normal((23, 11)) + 0.5
+    v, sums = O.mmd_l1(X, Y)
+    vp, _ = O.mmd_l1(X[rng.permutation(23)], Y[rng.permutation(23)])               # order of the elements
+    assert vp == pytest.approx(v, rel=1e-13)
+    vs, _ = O.mmd_l1(Y, X)                                                         # symmetric in (X, Y)
+    assert vs == pytest.approx(v, rel=1e-13)
+    vt, _ = O.mmd_l1(X + 3.25, Y + 3.25)                                           # l1 is translation invariant
+    assert vt == pytest.approx(v, rel=1e-12)
+    vc, _ = O.mmd_l1(-2.5 * X, -2.5 * Y)                                           # and absolutely homogeneous
+    assert vc == pytest.approx(2.5 * v, rel=1e-13)
+    assert v > 0                                                                    # shifted sets are apart
+
+
+def test_mmd_against_an_independent_l1_distance_matrix():
+    from scipy.spatial.distance import cdist
+    rng = np.random.default_rng(2)
+    X, Y = rng.random((40, 32)), rng.random((40, 32)) ** 2
+    v, sums = O.mmd_l1(X, Y)
+    dxy, dxx, dyy = cdist(X, Y, "cityblock"), cdist(X, X, "cityblock"), cdist(Y, Y, "cityblock")
+    assert sums[0] == pytest.approx(dxy.sum(), rel=1e-13) and sums[1] == pytest.approx(dxx.sum(), rel=1e-13)
+    assert v == pytest.approx((2 * dxy - dxx - dyy).mean(), rel=1e-12)
+
+
+def test_16bit_rounding_helpers():
+    """round_f16 / round_bf16 (expected values of the 16-bit output formats): round to nearest even on the format's grid."""
+    x = np.array([1.0, 1.0 + 2.0 ** -11, 1.0 + 3 * 2.0 ** -11, 0.1, -0.33333, 1.125, 2.0 ** -20])
+    assert list(O.round_f16(x)[:3]) == [1.0, 1.0, 1.0 + 2.0 ** -9]                 # ties go to the even code
+    assert list(O.round_bf16(np.array([1.0, 1.0 + 2.0 ** -8, 1.0 + 3 * 2.0 ** -8]))) == [1.0, 1.0, 1.0 + 2.0 ** -6]
+    for f, bits in ((O.round_f16, 11), (O.round_bf16, 8)):
+        r = f(x).astype(np.float64)
+        assert np.all(np.abs(r - x) <= np.abs(x) * 2.0 ** -bits)                   # within half an ulp
+        assert np.array_equal(f(r), r.astype(np.float32))                          # idempotent
