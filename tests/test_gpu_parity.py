@@ -120,7 +120,8 @@ def test_phase_c1(T):
             r = O.render_voice(u[b], nk[b], wl.sr, wl.N, neb, want_phase=True)
             d = np.abs(ph[b] - r[f"phase{vco}"])
             d = np.minimum(d, 1 - d)
-            # the audio kernel accumulates phase on a 2^-32 (VCO 1) / 2^-33 (VCO 2) cycle grid: <= 20 * 2^-33 per run
+            # the audio kernel accumulates phase on a 2^-32 (VCO 1) / 2^-33 (VCO 2) cycle grid: one rounding of at most
+            # 2^-33 cycle per add, 20 adds per run => <= 20 * 2^-33 = 2.3e-9 cycles, inside H4's 1e-8 budget
             assert d.max() < 3e-9, (vco, b, d.max())
 
 
@@ -144,13 +145,29 @@ def test_audio_c2_all_voices(T):
         assert not np.any(g[b, last:]), b
 
 
+def assert_parity_all_voices(T, dev, u, nk, wl, neb, what, chunk=256, full=None):
+    """Every voice of a full-size launch against the oracle, streamed in chunks of `chunk` voices to bound host memory
+    ("Parity on all voices ... stream voice by voice").  full: the [B, N] CUDA tensor already rendered."""
+    import torch
+    if full is None:
+        full = T.ts_render(dev, wl.sr, wl.seconds)                       # the bench's launch configuration: all voices
+    torch.cuda.synchronize()
+    worst = (0.0, 0.0, -1)
+    obuf = np.empty((chunk, wl.N), dtype=np.float64)
+    for b0 in range(0, wl.B, chunk):
+        nb = min(chunk, wl.B - b0)
+        g = full[b0:b0 + nb].cpu().numpy()
+        o = O.render_batch(u[b0:b0 + nb], nk[b0:b0 + nb], wl.sr, wl.N, neb, out=obuf[:nb])
+        w = assert_parity(g, o, f"{what} voices {b0}..")
+        if w[0] > worst[0]:
+            worst = (w[0], w[1], b0 + w[2])
+    return worst
+
+
 @pytest.mark.parametrize("batch", [0, 49, 99])
-def test_audio_c3_batches_sampled_voices(T, batch):
-    voices = np.arange(0, 1024, 16)
+def test_audio_c3_batches_all_voices(T, batch):
     wl, neb, u, nk, dev = setup_workload(T, "C3", batch_index=batch)
-    g = T.ts_render(dev, wl.sr, wl.seconds)[voices.tolist()].cpu().numpy()   # full-size launch, sampled rows
-    o = O.render_batch(u[voices], nk[voices], wl.sr, wl.N, neb)
-    print("C3 worst:", assert_parity(g, o, f"C3[{batch}]"))
+    print("C3 worst:", assert_parity_all_voices(T, dev, u, nk, wl, neb, f"C3[{batch}]"))
 
 
 def test_audio_c4_long_render_all_voices(T):
@@ -166,15 +183,10 @@ def test_audio_c4_long_render_all_voices(T):
             assert min(d, 1 - d) < 1e-7, (b, n, d)
 
 
-def test_audio_c5_full_launch_sampled_voices(T):
-    import torch
-    voices = np.concatenate([np.arange(0, 4096, 32), np.arange(1, 4096, 64)])
+def test_audio_c5_all_voices(T):
+    """BASELINE.json configs[4]: all 4096 voices (7.2e8 samples) of one full-size launch, streamed through the oracle."""
     wl, neb, u, nk, dev = setup_workload(T, "C5")
-    full = T.ts_render(dev, wl.sr, wl.seconds)
-    g = full[torch.from_numpy(voices).cuda()].cpu().numpy()
-    del full
-    o = O.render_batch(u[voices], nk[voices], wl.sr, wl.N, neb)
-    print("C5 worst:", assert_parity(g, o, "C5"))
+    print("C5 worst:", assert_parity_all_voices(T, dev, u, nk, wl, neb, "C5"))
 
 
 # ---------------------------------------------------------------------------------- edge cases
@@ -333,23 +345,59 @@ def test_random_nebula_parity(T, seed):
         T.ts_set_nebula(None)
 
 
-def test_render_controls_c2_sampled_voices(T):
-    """The control-rate call on its own (Fig. 2 workload) at C2 size against the oracle's mixer rows."""
+def test_render_controls_c2_all_voices(T):
+    """The control-rate call on its own (Fig. 2 workload) at C2 size against the oracle's mixer rows: its own
+    launch mode (no oscillator stage), every voice, exact zeros after the voice has gone silent for good."""
+    import torch
     wl, neb, u, nk, dev = setup_workload(T, "C2")
-    ctl = T.ts_render_controls(dev, wl.sr, wl.seconds).cpu().numpy()
+    out = T.ts_render_controls(dev, wl.sr, wl.seconds)
+    ctl = out.cpu().numpy()
     assert ctl.shape == (wl.B, 5, O.num_ticks(wl.N))
-    for b in range(0, wl.B, 9):
+    for b in range(wl.B):
         E, L, M = O.controls(O.map_all(u[b], neb), wl.sr, wl.N)
         nz = np.flatnonzero(np.any(M != 0.0, axis=0))
         last = nz[-1] + 1 if nz.size else 0
         assert np.max(np.abs(ctl[b] - M)) < 1e-12, b
+        assert not np.any(ctl[b][:, last:]), b
+    # every element is written by the call itself (no memset): poison the buffer and render again, bitwise equal
+    out2 = torch.full_like(out, float("nan"))
+    lib = T.lib()
+    import ctypes as C
+    assert lib.ts_render_controls(C.c_void_p(dev.data_ptr()), wl.B, wl.sr, float(wl.seconds), C.c_void_p(out2.data_ptr())) == 0
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2)
+    # the audio path's own control rows (debug export) agree with it bit for bit where the voice is audible
+    dbg = T.ts_debug_controls(dev, wl.sr, wl.seconds).cpu().numpy()
+    for b in range(0, wl.B, 7):
+        nz = np.flatnonzero(np.any(ctl[b] != 0.0, axis=0))
+        last = nz[-1] + 1 if nz.size else 0
+        assert np.array_equal(dbg[b][:, :last], ctl[b][:, :last]), b
+
+
+@pytest.mark.parametrize("R", [1, 7, 441])
+def test_render_controls_other_tick_spacings(T, R):
+    """the audio-rate-control mode (R = 1: every sample is a tick) and other spacings, at C2's
+    length, against the oracle's controls_r.  R = 1 at C2 size is 176 401 ticks per voice (1389 chunks in the look-back
+    chain); 16 voices keep the fp64 output at 113 MB."""
+    wl, neb, u, nk, dev = setup_workload(T, "C2")
+    B = 16 if R == 1 else wl.B
+    ctl = T.ts_render_controls_r(dev[:B].contiguous(), wl.sr, wl.seconds, R).cpu().numpy()
+    K = O.num_ticks_r(wl.N, R)
+    assert ctl.shape == (B, 5, K) and T.ts_num_ticks_r(wl.N, R) == K
+    for b in range(B):
+        E, L, M = O.controls_r(O.map_all(u[b], neb), wl.sr, wl.N, R)
+        # the LFO phase is an exact integer scan on the GPU and a wrapped fp64 sum in the oracle (D21): over 176 400
+        # ticks the oracle's own rounding reaches 1e-11 cycles; rows are O(1)
+        assert np.max(np.abs(ctl[b] - M)) < (1e-10 if R == 1 else 1e-12), (b, np.max(np.abs(ctl[b] - M)))
+        nz = np.flatnonzero(np.any(M != 0.0, axis=0))
+        last = nz[-1] + 1 if nz.size else 0
         assert not np.any(ctl[b][:, last:]), b
 
 
 def test_c3_streaming_protocol_100_batches(T):
     """BASELINE.json configs[2]: 1024 voices x 4 s rendered over 100 consecutive batch indices, here in the bench's
     launch configuration (ts_corpus_render, two alternating output slots); the last two batches against the oracle
-    on sampled voices, records bit-exact."""
+    on every voice, records bit-exact."""
     import torch
     wl = W.WORKLOADS["C3"]
     T.ts_set_nebula(None)
@@ -357,7 +405,6 @@ def test_c3_streaming_protocol_100_batches(T):
     ar = torch.empty((2, wl.B, wl.N), device="cuda")
     T.ts_corpus_render(wl.seed, 0, wl.batches, wl.sr, wl.seconds, pr, ar)
     torch.cuda.synchronize()
-    voices = np.arange(5, 1024, 64)
     neb = O.default_nebula()
     for batch in (wl.batches - 2, wl.batches - 1):
         slot = batch % 2
@@ -365,7 +412,155 @@ def test_c3_streaming_protocol_100_batches(T):
         rec = pr[slot].cpu().numpy()
         assert np.array_equal(rec[:, :78].view(np.uint32), u.view(np.uint32))
         assert np.array_equal(np.ascontiguousarray(rec[:, 78:]).view(np.uint32), nk)
-        g = ar[slot][voices.tolist()].cpu().numpy()
-        o = O.render_batch(u[voices], nk[voices], wl.sr, wl.N, neb)
-        assert_parity(g, o, f"C3 stream[{batch}]")
+        assert_parity_all_voices(T, None, u, nk, wl, neb, f"C3 stream[{batch}]", full=ar[slot])
         assert T.ts_corpus_is_test(batch * wl.B) == O.corpus_is_test(batch * wl.B)
+
+
+# ---------------------------------------------------------------------------------- 16-bit output formats
+def ulp16(x, mant_bits):
+    """spacing of the 16-bit format (mant_bits explicit mantissa bits) at |x| (normal range)."""
+    e = np.floor(np.log2(np.maximum(np.abs(x), 2.0 ** -14)))
+    return 2.0 ** (e - mant_bits)
+
+
+@pytest.mark.parametrize("fmt_name,mant", [("f16", 10), ("bf16", 7)])
+@pytest.mark.parametrize("wname", ["C1", "C2"])
+def test_audio_16bit_formats(T, fmt_name, mant, wname):
+    """fp16 / bf16 output: the finished fp32 sample rounded once (RNE).  Expected value = the oracle's fp64 sample rounded
+    the same way; bound per sample: the fp32 path's 2e-3 plus half an ulp of the format at that magnitude (a sample
+    within 2e-3 of the oracle can round to a neighbouring code).  Exactly-silent tails stay exact zeros, and the 16-bit
+    render equals the fp32 render rounded (bitwise)."""
+    import torch
+    fmt = {"f16": T.TS_F16, "bf16": T.TS_BF16}[fmt_name]
+    wl, neb, u, nk, dev = setup_workload(T, wname)
+    g16 = T.ts_render_fmt(dev, wl.sr, wl.seconds, fmt)
+    g32 = T.ts_render(dev, wl.sr, wl.seconds)
+    assert torch.equal(g16, g32.to(g16.dtype))                               # one RNE rounding of the fp32 sample
+    g = g16.float().cpu().numpy().astype(np.float64)
+    o = O.render_batch(u, nk, wl.sr, wl.N, neb)
+    rnd = (O.round_f16 if fmt_name == "f16" else O.round_bf16)(o).astype(np.float64)
+    tol = MAX_ABS + 0.5 * ulp16(o, mant)
+    assert np.all(np.abs(g - o) <= tol)
+    assert np.all(np.abs(g - rnd) <= MAX_ABS + ulp16(o, mant))
+    frac_same = np.mean(g == rnd)                                            # most samples land on the oracle's own code
+    assert frac_same > (0.9 if fmt_name == "bf16" else 0.5), frac_same
+    for b in range(wl.B):
+        nzo = np.flatnonzero(o[b])
+        last = nzo[-1] + 1 if nzo.size else 0
+        assert not np.any(g[b, last:]), b
+
+
+@pytest.mark.parametrize("sr,seconds,B", [(44100, 0.0123, 3), (48000, 0.50001, 2), (44100, 2564 / 44100, 2)])
+def test_16bit_ragged_and_unaligned(T, sr, seconds, B):
+    import torch
+    T.ts_set_nebula(None)
+    u, nk = O.sample_params(3, 1, B)
+    N = O.num_samples(sr, seconds)
+    for off in (0, 1):                                                       # 1: rows only 2-byte aligned
+        pad = torch.full((B * N + 64 + off,), 7.0, device="cuda", dtype=torch.float16)
+        out = pad[off:off + B * N].view(B, N)
+        T.ts_render_fmt(to_dev(u, nk), sr, seconds, T.TS_F16, out=out)
+        assert torch.all(pad[off + B * N:] == 7.0) and torch.all(pad[:off] == 7.0)
+        ref = T.ts_render(to_dev(u, nk), sr, seconds)
+        assert torch.equal(out, ref.half())
+
+
+def test_render_host_fmt_and_corpus_fmt(T):
+    import torch
+    T.ts_set_nebula(None)
+    B, sr, seconds = 6, 44100, 0.4
+    N = O.num_samples(sr, seconds)
+    host = T.ts_render_host_fmt(4, 2, B, sr, seconds, T.TS_BF16)
+    p = T.ts_sample_params(4, 2, B)
+    assert torch.equal(host.cuda(), T.ts_render(p, sr, seconds).bfloat16())
+    pr = torch.zeros((3, B, 80), device="cuda")
+    ar = torch.zeros((3, B, N), device="cuda", dtype=torch.float16)
+    T.ts_corpus_render_fmt(4, 0, 5, sr, seconds, T.TS_F16, pr, ar)
+    torch.cuda.synchronize()
+    for i in (2, 3, 4):
+        q = T.ts_sample_params(4, i, B)
+        assert torch.equal(pr[i % 3].view(torch.int32), q.view(torch.int32))
+        assert torch.equal(ar[i % 3], T.ts_render(q, sr, seconds).half())
+
+
+# ---------------------------------------------------------------------------------- the corpus iterator (SURVEY 8(f) item 1)
+def test_corpus_iterator_hands_out_audio_params_and_split(T):
+    """ts_corpus_open / next / close: (audio, params, is_test) per batch, P:L94 / P:L98 / P:L102.  B = 128 at the paper's
+    default batch size; 1024 / 128 = 8 batches per block, so batches 72..79 are the first test block (g in [9216, 10240))."""
+    import torch
+    T.ts_set_nebula(None)
+    B, sr, seconds, first = 128, 44100, 0.25, 68
+    N = O.num_samples(sr, seconds)
+    for n_ring in (2, 3):
+        pr = torch.zeros((n_ring, B, 80), device="cuda")
+        ar = torch.full((n_ring, B, N), 9.0, device="cuda")
+        T.ts_corpus_open(0, first, sr, seconds, T.TS_F32, pr, ar)
+        got = []
+        for k in range(14):
+            b = T.ts_corpus_next()
+            assert b["batch_index"] == first + k and b["first_voice"] == (first + k) * B and b["slot"] == (first + k) % n_ring
+            want_test = O.corpus_is_test(b["first_voice"])
+            assert b["is_test_first"] == want_test == b["is_test_last"] == (72 <= first + k < 80)
+            got.append((b["audio"].clone(), b["params"].clone()))            # consumed on the current stream
+        T.ts_corpus_close()
+        torch.cuda.synchronize()
+        for k in (0, 5, 13):
+            p = T.ts_sample_params(0, first + k, B)
+            assert torch.equal(got[k][1].view(torch.int32), p.view(torch.int32))
+            assert torch.equal(got[k][0], T.ts_render(p, sr, seconds))
+    u, nk = O.sample_params(0, first + 13, B)                                # and against the oracle
+    assert_parity(got[13][0].cpu().numpy(), O.render_batch(u, nk, sr, N), "iterator")
+    with pytest.raises(T.TsynthError):
+        T.ts_corpus_next()                                                   # closed
+
+
+# ---------------------------------------------------------------------------------- Eq. 2: MMD with the l1 core distance (SURVEY 8(f) item 4)
+@pytest.mark.parametrize("n,d", [(1000, 512), (37, 5), (64, 32), (129, 100), (1, 3)])
+def test_mmd_l1_against_oracle(T, n, d):
+    """The paper's setting (n = 1000 sounds, d = 512 OpenL3 values) and ragged sizes.  Differences and per-pair
+    sums are fp32 on the GPU (inputs O(1): each |x - y| carries 2^-24 relative, a pair sum over d terms at most
+    d 2^-24 relative), pair sums are added in fp64: 1e-5 relative on each of the three sums covers d = 512 with margin."""
+    import torch
+    rng = np.random.default_rng(n * 1000 + d)
+    X = rng.standard_normal((n, d)).astype(np.float32)
+    Y = (0.7 * rng.standard_normal((n, d)) + 0.3).astype(np.float32)
+    out = T.ts_mmd_l1(torch.from_numpy(X).cuda(), torch.from_numpy(Y).cuda()).cpu().numpy()
+    v, sums = O.mmd_l1(X, Y)
+    for k in range(3):
+        assert out[1 + k] == pytest.approx(sums[k], rel=1e-5)
+    scale = max(sums[0], 1.0) / (n * n)
+    assert abs(out[0] - v) <= 4e-5 * scale, (out[0], v)
+    same = T.ts_mmd_l1(torch.from_numpy(X).cuda(), torch.from_numpy(X).cuda()).cpu().numpy()
+    assert same[0] == 0.0 and same[1] == same[2] == same[3]                  # MMD(X, X) = 0 exactly
+    again = T.ts_mmd_l1(torch.from_numpy(X).cuda(), torch.from_numpy(Y).cuda()).cpu().numpy()
+    assert np.array_equal(out, again)                                        # fixed summation order
+
+
+# ---------------------------------------------------------------------------------- legal end-of-range LFO inputs (H8)
+def test_end_of_range_lfo_inputs_stay_finite_and_agree_off_the_jumps(T):
+    """LFO rate / depth / start phase at the ENDS of their ranges (30 Hz at cr = 441 Hz from phase 0.5 lands exactly on
+    the saw / square jump every 147 ticks: the side taken there is decided by the last rounding, reading H8).  Both
+    sides must stay finite everywhere, and agree on every control interval whose two ticks are away from a jump."""
+    T.ts_set_nebula(None)
+    rng = np.random.default_rng(5)
+    B, sr, seconds = 8, 44100, 1.0
+    u, nk = O.sample_params(21, 0, B)
+    for idx in (32, 33, 34, 40, 41, 42):
+        u[:, idx] = rng.integers(0, 2, size=B).astype(np.float32)
+    N = O.num_samples(sr, seconds)
+    g = T.ts_render(to_dev(u, nk), sr, seconds).cpu().numpy()
+    gc = T.ts_debug_controls(to_dev(u, nk), sr, seconds).cpu().numpy()
+    assert np.all(np.isfinite(g)) and np.all(np.isfinite(gc)) and np.abs(g).max() <= 1.2
+    for b in range(B):
+        o = O.render_voice(u[b], nk[b], sr, N)["audio"]
+        E, L, M = O.controls(O.map_all(u[b]), sr, N)
+        assert np.all(np.isfinite(o))
+        bad_tick = np.any(np.abs(gc[b] - M) > 1e-9, axis=0)                  # ticks where the two sides took different sides
+        K = M.shape[1]
+        ok_iv = ~(bad_tick[:-1] | bad_tick[1:])                              # intervals with both ticks in agreement
+        # pitch rows feed the phase: after the first flipped interval the phases differ, so compare up to there
+        first_bad = int(np.argmin(ok_iv)) if not ok_iv.all() else K - 1
+        n_ok = min(N, first_bad * 100)
+        if n_ok > 0:
+            d = g[b, :n_ok].astype(np.float64) - o[:n_ok]
+            assert np.abs(d).max() <= MAX_ABS, (b, first_bad, np.abs(d).max())
