@@ -1,11 +1,13 @@
 #!/usr/bin/env python
-"""bench.py -- throughput of the whole hot path (sampler -> control -> audio) on synthetic workloads.
+"""bench.py -- throughput of the whole hot path (sampler -> setup -> control -> audio) on synthetic workloads.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--repeats R] [--workload C2] [--impl ours|reference]
 
-A step = one batch of the workload (BASELINE.json configs[1] = C2 by default: 128 voices x 4 s at 44.1 kHz)
-through ts_sample_params + ts_render, batch index = the step number (streaming corpus generation).
-Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle on the host cores instead.
+A step = one batch of the workload (BASELINE.json configs[1] = C2 by default: 128 voices x 4 s at 44.1 kHz) through the
+streaming call ts_corpus_render, batch index = the step number (streaming corpus generation).  The K-step timed
+region is repeated R times (each bracketed by a barrier and a device synchronisation); `value` is the median region.
+Prints ONE JSON line (rank 0).  `--gpus N` outside torchrun starts the N ranks itself.  `--impl reference` times the CPU
+oracle on the host cores instead.
 """
 from __future__ import annotations
 
@@ -23,6 +25,11 @@ sys.path.insert(0, ROOT)
 METRIC = "audio samples/sec"
 UNIT = "samples/s"
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
+# Measured saturated throughput of the audible-sample instruction mix (the kernel's own loop body, no memory, 8 warps per
+# SM sub-partition; profiles/r02_audio_bounds.md): cycles per warp-unit of 640 samples per sub-partition.
+BODY_CYCLES_PER_UNIT = 1082.0
+UNIT_SAMPLES = 640
+SMSPS = 148 * 4
 
 
 def measured_peak():
@@ -36,8 +43,7 @@ def measured_peak():
 
 def ncu_value(name: str, workload: str):
     """A per-launch counter of the audio kernel from the committed summary of the latest `ncu --set full` capture
-    (profiles/<name>.csv: workload,value), if any.  audio_kernel_traffic = dram__bytes_read.sum +
-    dram__bytes_write.sum; audio_kernel_warp_instructions = smsp__inst_executed.sum."""
+    (profiles/<name>.csv: workload,value), if any.  audio_kernel_traffic = dram__bytes_read.sum + dram__bytes_write.sum."""
     p = os.path.join(ROOT, "profiles", name + ".csv")
     try:
         with open(p) as f:
@@ -48,6 +54,17 @@ def ncu_value(name: str, workload: str):
     except Exception:
         pass
     return None
+
+
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
 
 
 class ClockSampler:
@@ -128,7 +145,7 @@ def run_reference(args, wl):
     t0 = time.perf_counter()
     total = 0
     for _ in range(args.steps):
-        v, _dt = oracle_samples_per_s(wl, voices, 1, cores)
+        oracle_samples_per_s(wl, voices, 1, cores)
         total += voices * wl.N
     dt = time.perf_counter() - t0
     value = total / dt
@@ -139,9 +156,94 @@ def run_reference(args, wl):
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"{wl.name}: B={wl.B} x {wl.seconds} s @ {wl.sr} Hz (oracle on a bounded sample: {sample})"},
         "x_real_time": value / wl.sr,
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "cpu_model": cpu_model()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
+
+
+def device_records(ts, W, wl, dev):
+    """The workload's parameter records on the device: the GPU's own draw, host-side edits of u (inputs, not method
+    arithmetic: workloads.py) applied once and uploaded."""
+    import torch
+    rec = ts.ts_sample_params(wl.seed, 0, wl.B, device=dev)
+    if wl.edit == "none":
+        return rec
+    h = rec.cpu().numpy()
+    h[:, :78] = W.edit_u(h[:, :78], wl, 0)
+    return torch.from_numpy(h).to(dev)
+
+
+def kernel_roofline(ts, wl, rec, audio_ring, sm_hz, reps):
+    """Per-kernel device times (CUDA events around `reps` back-to-back launches of each, ts_time_kernels), the active
+    (non-silent) sample fraction, and the two bounds of the audio kernel."""
+    B, sr, seconds, N = wl.B, wl.sr, wl.seconds, wl.N
+    ctl, aud = ts.ts_time_kernels(rec, sr, seconds, audio_ring, reps)
+    ts.ts_set_timing(True)
+    ts.ts_render(rec, sr, seconds, out=audio_ring[0])
+    ts.ts_sync()                                   # the active-sample count is valid after ts_sync
+    stats = ts.ts_last_stats()
+    ts.ts_set_timing(False)
+    active = stats["active_samples"] / float(B * N)
+    peak, peak_src = measured_peak()
+    out_bytes = B * N * 4
+    achieved = out_bytes / (aud * 1e-3) / 1e9
+    alu_peak = SMSPS * UNIT_SAMPLES / BODY_CYCLES_PER_UNIT * sm_hz          # audible samples/s the SMs can compute
+    alu_ach = stats["active_samples"] / (aud * 1e-3)
+    return {"audio_kernel_ms": aud, "control_kernel_ms": ctl, "achieved_gbs": achieved, "frac": achieved / peak,
+            "peak": peak, "peak_source": peak_src, "active_sample_fraction": active, "chunks": stats["chunks"],
+            "alu_bound": {"bound": "alu", "what": "audible samples/s at the measured saturated throughput of the kernel's own "
+                          "instruction mix (1082 cycles per 640-sample warp-unit per SM sub-partition, 592 sub-partitions; "
+                          "profiles/r02_audio_bounds.md)", "achieved": alu_ach, "peak": alu_peak, "unit": "audible samples/s",
+                          "frac": alu_ach / alu_peak}}
+
+
+def measure_config(ts, W, torch, name, dev, sm_hz):
+    """One extra workload (C1, C3, C4, C5) on rank 0: whole-path step time (median and best of 5 regions) and the audio
+    kernel's roofline numbers.  C3 streams consecutive batch indices through ts_corpus_render (sampler included); C4 / C5
+    render the same edited records repeatedly through ts_render (setup + control + audio; the 2.5 us sampler is not in
+    their step)."""
+    wl = W.WORKLOADS[name]
+    B, sr, seconds, N = wl.B, wl.sr, wl.seconds, wl.N
+    ts.ts_set_nebula(W.apply_nebula(ts.ts_default_nebula(), wl))
+    out_bytes = B * N * 4
+    nbuf = min(256, max(2, -(-(160 << 20) // out_bytes) + 1))
+    audio_ring = torch.empty((nbuf, B, N), dtype=torch.float32, device=dev)
+    rec = device_records(ts, W, wl, dev)
+    steps = max(3, min(200, int(0.02 / (out_bytes / 2.0e12))))       # ~20 ms of device time per region
+    regions = []
+    if wl.edit == "none":
+        params_ring = torch.empty((nbuf, B, 80), dtype=torch.float32, device=dev)
+        ts.ts_corpus_render(wl.seed, 0, 3, sr, seconds, params_ring, audio_ring)
+        how = "ts_corpus_render over consecutive batch indices (sampler + setup + control + audio)"
+    else:
+        for k in range(3):
+            ts.ts_render(rec, sr, seconds, out=audio_ring[k % nbuf])
+        how = "ts_render on the edited records (setup + control + audio)"
+    torch.cuda.synchronize()
+    for r in range(5):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        if wl.edit == "none":
+            ts.ts_corpus_render(wl.seed, 3 + r * steps, steps, sr, seconds, params_ring, audio_ring)
+        else:
+            for k in range(steps):
+                ts.ts_render(rec, sr, seconds, out=audio_ring[k % nbuf])
+        e1.record()
+        torch.cuda.synchronize()
+        regions.append(e0.elapsed_time(e1) / steps)
+    med, best = statistics.median(regions), min(regions)
+    roof = kernel_roofline(ts, wl, rec, audio_ring, sm_hz, 20 if out_bytes < (200 << 20) else 4)
+    sps = B * N / (med * 1e-3)
+    res = {"workload": f"{name}: B={B} voices x {seconds} s @ {sr} Hz", "how": how, "steps_per_region": steps, "regions": 5,
+           "ms_per_step": med, "ms_per_step_best": best, "samples_per_s": sps, "x_real_time": sps / sr,
+           "audible_samples_per_s": sps * roof["active_sample_fraction"],
+           "audio_kernel_ms": roof["audio_kernel_ms"], "control_kernel_ms": roof["control_kernel_ms"], "frac": roof["frac"],
+           "alu_bound_frac": roof["alu_bound"]["frac"], "active_sample_fraction": roof["active_sample_fraction"],
+           "step_over_audio_kernel": med / roof["audio_kernel_ms"], "voice_chunks_per_launch": roof["chunks"]}
+    del audio_ring
+    torch.cuda.empty_cache()
+    return res
 
 
 def run_ours(args, wl):
@@ -150,128 +252,153 @@ def run_ours(args, wl):
     from paper_2104_12922_b200 import build, shard, workloads as W
     build.build()
     rank, local_rank, world = shard.init("nccl")
+    if world != args.gpus:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE is {world}")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     B, sr, seconds, N = wl.B, wl.sr, wl.seconds, wl.N
-    ts.ts_set_nebula(W.apply_nebula(ts.ts_default_nebula(), wl))
     if wl.edit != "none":
-        raise SystemExit("bench workloads with host-side parameter edits are parity-test cases (C4, C5): use C2 or C3")
+        raise SystemExit("the headline workload streams batch indices (C1, C2, C3); C4 / C5 are reported under `configs`")
+    ts.ts_set_nebula(W.apply_nebula(ts.ts_default_nebula(), wl))
 
     # rotating output buffers: together larger than the 126 MB L2, so no step rewrites lines still cached
     out_bytes = B * N * 4
-    nbuf = max(2, -(-(160 << 20) // out_bytes) + 1)
+    nbuf = min(256, max(2, -(-(160 << 20) // out_bytes) + 1))
     audio_ring = torch.empty((nbuf, B, N), dtype=torch.float32, device=dev)
     params_ring = torch.empty((nbuf, B, 80), dtype=torch.float32, device=dev)
-    outs = [audio_ring[k] for k in range(nbuf)]
-    params = [params_ring[k] for k in range(nbuf)]
 
-    def step(i):        # one batch through the two plain calls (used for the per-kernel timings below)
-        k = i % nbuf
-        ts.ts_sample_params(wl.seed, shard.batch_index(i, rank, world), B, out=params[k])
-        ts.ts_render(params[k], sr, seconds, out=outs[k])
-
-    # the timed region: K consecutive batch indices of this rank through the streaming call (ts_corpus_render:
-    # sampler -> control -> audio per batch, consecutive batches on two internal streams)
-    first = rank * (args.warmup + args.steps)
-    ts.ts_corpus_render(wl.seed, first, args.warmup, sr, seconds, params_ring, audio_ring)
+    # ---- the timed regions: K consecutive batch indices of this rank's contiguous range through the streaming call
+    # (sampler + setup + control + audio per batch, consecutive batches on two internal streams), R times
+    K, Wm, R = args.steps, args.warmup, args.repeats
+    per_rank = Wm + K * R
+    first, _count = shard.batch_range(rank, world, per_rank)
+    ts.ts_corpus_render(wl.seed, first, Wm, sr, seconds, params_ring, audio_ring)
     torch.cuda.synchronize()
-    shard.barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    regions = []
+    launches = 0
     with ClockSampler(local_rank) as clk:
-        torch.cuda.synchronize()
-        e0.record()
-        ts.ts_corpus_render(wl.seed, first + args.warmup, args.steps, sr, seconds, params_ring, audio_ring)
-        e1.record()
-        torch.cuda.synchronize()
-    shard.barrier()
-    ms = shard.max_over_ranks(e0.elapsed_time(e1), dev)
-    total_samples = float(B) * N * args.steps * world
+        for r in range(R):
+            shard.barrier()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ts.ts_corpus_render(wl.seed, first + Wm + r * K, K, sr, seconds, params_ring, audio_ring)
+            e1.record()
+            torch.cuda.synchronize()
+            shard.barrier()
+            regions.append(shard.max_over_ranks(e0.elapsed_time(e1), dev))
+            launches = ts.ts_last_stats()["launches"]
+    ms = statistics.median(regions)
+    total_samples = float(B) * N * K * world
     value = total_samples / (ms * 1e-3)
     clocks = clk.summary()
-    if clocks["samples"] < 5 and clk.nv:          # timed region too short for NVML: same load, untimed, 0.3 s
-        with ClockSampler(local_rank) as clk2:
-            t0 = time.perf_counter()
-            i = 0
-            while time.perf_counter() - t0 < 0.3:
-                step(i)
-                i += 1
-            torch.cuda.synchronize()
-        clocks = clk2.summary()
-        clocks["note"] = "timed region shorter than the NVML poll; sampled on the same loop run for 0.3 s"
+    sm_hz = 1e6 * float(clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965)
 
     # ---- roofline of the dominant kernel (audio): algorithmic bytes = 4 B per output sample
-    # (a) average launch duration over back-to-back launches (CUDA events on the library's stream around 50 launches
-    #     of each kernel, outputs rotating over the ring); (b) one isolated launch bracketed by its own event pair,
-    #     which adds the ~6 us an empty kernel shows between two events on this box.
-    reps = 50
-    ctl, aud = ts.ts_time_kernels(params[0], sr, seconds, audio_ring, reps)
-    ts.ts_set_timing(True)
-    ctl_1, aud_1 = [], []
-    for i in range(10):
-        step(i)
-        c, a = ts.ts_last_kernel_ms()
-        ctl_1.append(c)
-        aud_1.append(a)
-    stats = ts.ts_last_stats()
-    launches_per_step = 1 + stats["launches"]
-    active_frac = stats["active_samples"] / float(B * N)
-    ts.ts_set_timing(False)
-    torch.cuda.synchronize()
-    peak, peak_src = measured_peak()
-    achieved = out_bytes / (aud * 1e-3) / 1e9
+    rec = device_records(ts, W, wl, dev)
+    roof = kernel_roofline(ts, wl, rec, audio_ring, sm_hz, 50)
+    fill_ms = ts.ts_time_fill(audio_ring, 5)
+    fill_gbs = audio_ring.numel() * 4 / (fill_ms * 1e-3) / 1e9
     traffic = ncu_value("audio_kernel_traffic", wl.name)
-    winst = ncu_value("audio_kernel_warp_instructions", wl.name)
-    sm_hz = 1e6 * float(clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965)
-    issue = None
-    if winst:       # the other bound of this kernel: 148 SMs x 4 schedulers x 1 warp instruction per clock
-        ipeak = 148 * 4 * sm_hz
-        issue = {"bound": "alu", "what": "warp-instruction issue slots", "achieved": winst / (aud * 1e-3), "peak": ipeak,
-                 "unit": "warp-instructions/s", "frac": winst / (aud * 1e-3) / ipeak,
-                 "warp_instructions_per_launch": winst}
-    roofline = {"bound": "hbm", "kernel": "ts_audio_kernel<0>", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": out_bytes, "audio_kernel_ms": aud, "control_kernel_ms": ctl,
-                "timing": f"CUDA events around {reps} back-to-back launches of each kernel (ts_time_kernels)",
-                "isolated_launch_ms": {"audio": statistics.mean(aud_1), "control": statistics.mean(ctl_1)},
-                "active_sample_fraction": active_frac, "issue_bound": issue,
-                "note": "audible samples are issue-bound (~46 SASS instructions each), silent tails are pure stores; "
-                        "see DESIGN.md 5.2 for the issue-slot bound stated beside this HBM one",
-                "whole_step_frac_of_write_roofline": (4.0 * value / world / 1e9) / peak}
+    roofline = {"bound": "hbm", "kernel": "ts_audio_kernel<0, TAIL, F32>", "achieved": roof["achieved_gbs"], "peak": roof["peak"],
+                "unit": "GB/s", "frac": roof["frac"], "traffic": traffic,
+                "traffic_source": "stored value: dram__bytes_read.sum + dram__bytes_write.sum of one launch in the committed "
+                                  "`ncu --set full` capture (profiles/audio_kernel_traffic.csv), not measured in this run; it is "
+                                  "below the algorithmic bytes because the 126 MB L2 still holds the end of a single launch's writes",
+                "peak_source": roof["peak_source"], "algorithmic_bytes_per_launch": out_bytes,
+                "audio_kernel_ms": roof["audio_kernel_ms"], "control_kernel_ms": roof["control_kernel_ms"],
+                "timing": "CUDA events around 50 back-to-back launches of each kernel (ts_time_kernels); control = setup + control",
+                "store_only_fill_gbs": fill_gbs,
+                "store_only_fill": f"{audio_ring.numel() * 4 >> 20} MiB of 128-bit zero stores, 5 launches (ts_time_fill): what a pure "
+                                   "store stream reaches, beside the copy peak above",
+                "active_sample_fraction": roof["active_sample_fraction"], "alu_bound": roof["alu_bound"],
+                "note": "audible samples are bound by the SM pipes (FMA-heavy: Philox IMAD.WIDE + packed fp32; ~46 SASS instructions "
+                        "each), silent tails are pure stores written asynchronously by the audible CTAs; DESIGN.md 5.2 and "
+                        "profiles/r02_audio_bounds.md state the measured ALU bound beside this HBM one",
+                "whole_step_frac_of_write_roofline": (4.0 * value / world / 1e9) / roof["peak"]}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32 (audio) + f64 / Q0.64 (control and phase chain)", "data": "synthetic",
-            "config": {"workload": f"{wl.name}: B={B} voices x {seconds} s @ {sr} Hz per GPU per step, seed 0, consecutive batch indices "
-                                   "through ts_corpus_render (sampler + control + audio per batch)",
-                       "l2": f"{nbuf} rotating output buffers of {out_bytes >> 20} MiB (> 126 MB L2 together)"},
-            "x_real_time": value / sr, "clocks": clocks, "gpu_launches": launches_per_step * args.steps,
+            "config": {"workload": f"{wl.name}: B={B} voices x {seconds} s @ {sr} Hz per GPU per step, seed 0, consecutive batch "
+                                   "indices through ts_corpus_render (sampler + setup + control + audio per batch)",
+                       "l2": f"{nbuf} rotating output buffers of {out_bytes >> 20} MiB (> 126 MB L2 together)",
+                       "partition": f"rank r renders the contiguous batch-index range [r*{per_rank}, (r+1)*{per_rank})"},
+            "timing": {"repeats": R, "ms_per_step_median": ms / K, "ms_per_step_best": min(regions) / K,
+                       "ms_per_step_all": [x / K for x in regions],
+                       "how": "each repeat = exactly K steps between two CUDA events, barrier + synchronize on both sides, max over ranks"},
+            "x_real_time": value / sr, "audible_samples_per_s": value * roof["active_sample_fraction"],
+            "step_over_audio_kernel": (ms / K) / roof["audio_kernel_ms"],
+            "clocks": clocks, "gpu_launches": int(launches) * world,
             "roofline": roofline,
             "paper_context": "714e6 samples/s on one V100 (P:L23); other hardware, context only"}
 
-    # ---- end to end through the public host-buffer call: sample + render + D2H of audio and records
+    # ---- end to end through the public host-buffer call: sample + render + D2H of audio and records, fp32 and fp16
     if rank == 0 or world > 1:
-        host = torch.empty((B, N), dtype=torch.float32, pin_memory=True)
-        hostp = torch.empty((B, 80), dtype=torch.float32, pin_memory=True)
-        n_e2e = max(3, min(args.steps, 10))
-        ts.ts_render_host(wl.seed, 0, B, sr, seconds, host, hostp)
-        shard.barrier()
-        t0 = time.perf_counter()
-        for i in range(n_e2e):
-            ts.ts_render_host(wl.seed, shard.batch_index(i, rank, world), B, sr, seconds, host, hostp)
-        dt = shard.max_over_ranks(time.perf_counter() - t0, dev)
-        line["e2e"] = {"value": float(B) * N * n_e2e * world / dt, "unit": UNIT, "h2d_bytes_per_step": 0,
-                       "d2h_bytes_per_step": out_bytes + B * 320, "steps": n_e2e,
-                       "note": "inputs are (seed, batch index) scalars: nothing to copy host->device"}
+        n_e2e = max(3, min(K, 10))
+        first_e2e, _ = shard.batch_range(rank, world, n_e2e + 1)
+        for key, fmt, dt, es in (("e2e", ts.TS_F32, torch.float32, 4), ("e2e_f16", ts.TS_F16, torch.float16, 2)):
+            host = torch.empty((B, N), dtype=dt, pin_memory=True)
+            hostp = torch.empty((B, 80), dtype=torch.float32, pin_memory=True)
+            ts.ts_render_host_fmt(wl.seed, first_e2e, B, sr, seconds, fmt, host, hostp)
+            shard.barrier()
+            t0 = time.perf_counter()
+            for i in range(n_e2e):
+                ts.ts_render_host_fmt(wl.seed, first_e2e + 1 + i, B, sr, seconds, fmt, host, hostp)
+            dt_s = shard.max_over_ranks(time.perf_counter() - t0, dev)
+            line[key] = {"value": float(B) * N * n_e2e * world / dt_s, "unit": UNIT, "h2d_bytes_per_step": 0,
+                         "d2h_bytes_per_step": B * N * es + B * 320, "steps": n_e2e,
+                         "note": "inputs are (seed, batch index) scalars: nothing to copy host->device; PCIe-bound on the audio copy"}
 
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cores = os.cpu_count() or 1
-        voices = min(wl.B, 128)
-        _v, dt1 = oracle_samples_per_s(wl, voices, 1, cores)
-        repeats = max(2, min(400, int(15.0 / max(dt1, 1e-3))))           # ~15 s of wall clock on all cores
-        v, dt = oracle_samples_per_s(wl, voices, repeats, cores)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"first {voices} voices of the batch x {seconds} s, {repeats} repeats, "
-                                          f"{dt:.1f} s wall on {cores} threads"}
+    if rank == 0 and world == 1:
+        # ---- the other configs (BASELINE.json configs[0], [2..4]) beside the headline, so that it is not a memset number
+        if not args.no_configs:
+            line["configs"] = {name: measure_config(ts, W, torch, name, dev, sm_hz) for name in ("C1", "C3", "C4", "C5") if name != wl.name}
+            ts.ts_set_nebula(W.apply_nebula(ts.ts_default_nebula(), wl))
+        # ---- control-rate call on its own, MMD arithmetic
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ctl_out = ts.ts_render_controls(rec, sr, seconds)
+        torch.cuda.synchronize()
+        e0.record()
+        lib = ts.lib()
+        import ctypes as C
+        for _ in range(20):
+            lib.ts_render_controls(C.c_void_p(rec.data_ptr()), B, sr, float(seconds), C.c_void_p(ctl_out.data_ptr()))
+        e1.record()
+        torch.cuda.synchronize()
+        line["controls_only"] = {"ms_per_call": e0.elapsed_time(e1) / 20, "what": f"ts_render_controls on {wl.name}: {B} voices x "
+                                 f"{ctl_out.shape[2]} ticks x 5 rows fp64 (setup + control kernel without the oscillator stage)"}
+        n, d = 1000, 512
+        g = torch.Generator(device=dev).manual_seed(0)
+        X = torch.randn((n, d), device=dev, generator=g)
+        Y = 0.7 * torch.randn((n, d), device=dev, generator=g) + 0.3
+        ts.ts_mmd_l1(X, Y)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(20):
+            ts.ts_mmd_l1(X, Y)
+        e1.record()
+        torch.cuda.synchronize()
+        mmd_ms = e0.elapsed_time(e1) / 20
+        T = -(-n // 64)
+        pair_comps = (T * T + T * (T + 1)) * 64 * 64 * d                 # (pair, component) items computed, padded tiles included
+        alu_s = 2.0 * pair_comps / (148 * 128 * sm_hz)                    # 2 FADD-class thread instructions per item
+        line["mmd_l1"] = {"ms_per_call": mmd_ms, "n": n, "d": d, "bound": "alu", "unit": "s",
+                          "peak_s": alu_s, "frac": alu_s / (mmd_ms * 1e-3),
+                          "what": "Eq. 2 with the l1 core distance (P:L230); bound = 2 FADD-class instructions per (pair, component) "
+                                  "at 148 SMs x 128 fp32 lanes per clock; embeddings (4 MB) are L2-resident"}
+        if not args.no_cpu_baseline:
+            cores = os.cpu_count() or 1
+            voices = min(wl.B, 128)
+            _v, dt1 = oracle_samples_per_s(wl, voices, 1, cores)
+            repeats = max(2, min(400, int(12.0 / max(dt1, 1e-3))))           # ~12 s of wall clock on all cores
+            v, dt = oracle_samples_per_s(wl, voices, repeats, cores)
+            v1, dts = oracle_samples_per_s(wl, 8, 2, 1)                       # and one thread: 8 voices twice
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"first {voices} voices of the batch x {seconds} s, {repeats} repeats, "
+                                              f"{dt:.1f} s wall on {cores} threads",
+                                    "one_thread": {"value": v1, "unit": UNIT, "sample": f"8 voices x {seconds} s twice, {dts:.1f} s"},
+                                    "x_real_time": v / sr, "cpu_model": cpu_model()}
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
@@ -282,19 +409,25 @@ def run_ours(args, wl):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--repeats", type=int, default=21, help="timed regions of exactly --steps steps; value = the median one")
     ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the C1 / C3 / C4 / C5 entries of the line")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
-    from paper_2104_12922_b200 import workloads as W
+    args.repeats = max(args.repeats, 1)
+    from paper_2104_12922_b200 import shard, workloads as W
     wl = W.WORKLOADS[args.workload]
     if args.impl == "reference":
         run_reference(args, wl)
-    else:
-        run_ours(args, wl)
+        return
+    if args.gpus > 1 and not shard.under_torchrun():
+        # `python bench.py --gpus N` without a torchrun environment: start the N ranks ourselves
+        sys.exit(shard.respawn_under_torchrun(args.gpus, os.path.abspath(__file__), sys.argv[1:]))
+    run_ours(args, wl)
 
 
 if __name__ == "__main__":

@@ -152,7 +152,8 @@ int chunk_voices(int B, int K) {
     size_t c = TS_TABLE_BUDGET / per;
     if (c < 1) c = 1;
     if (c > (size_t)B) c = (size_t)B;
-    return (int)c;
+    const size_t n = ((size_t)B + c - 1) / c;  // chunks needed; spread the voices evenly over them
+    return (int)(((size_t)B + n - 1) / n);
 }
 struct ws_layout_t {
     size_t off_hdr, off_vc, off_agg, agg_bytes, total;
@@ -363,28 +364,76 @@ int fork_streams() {
     return TS_OK;
 }
 
-// One batch of the streaming path on the internal streams: records drawn and set up on `hi`, audio on `lo`.
-int stream_batch(uint64_t seed, uint64_t batch, int B, int sr, double seconds, int fmt, ts_voice *p, void *a) {
-    ts_lane &L = S.lane[1 + (int)(S.stream_count++ & 1)];
-    S.cur = &L;
+// A batch on the internal streams (forked by the caller): the voice chunks of the batch alternate between the two
+// streaming lanes, setup + control on `hi`, audio on `lo`, so that the control stage of one chunk overlaps the audio
+// stage of the previous one -- across the chunks of a batch as well as across batches.
+int stream_batch(ts_voice *p, sample_spec smp, int B, int sr, double seconds, int fmt, void *a, float *params_human) {
+    int64_t N;
+    int K;
+    int rc = check_sizes(B, sr, seconds, &N, &K);
+    if (rc) return rc;
+    const int Bc = chunk_voices(B, K);
+    const size_t es = fmt_bytes(fmt);
     const bool timing = S.timing;
     S.timing = false;  // per-kernel events would serialise the streams
-    const int rc = render_impl(p, sample_spec{true, seed, batch * (uint64_t)B}, B, sr, seconds, fmt, a, nullptr, 0, nullptr);
+    int64_t launches = 0, chunks = 0;
+    for (int b0 = 0; b0 < B && rc == TS_OK; b0 += Bc) {
+        const int nb = (B - b0 < Bc) ? (B - b0) : Bc;
+        S.cur = &S.lane[1 + (int)(S.stream_count++ & 1)];
+        rc = render_impl(p + b0, sample_spec{smp.on, smp.seed, smp.g0 + (uint64_t)b0}, nb, sr, seconds, fmt,
+                         static_cast<char *>(a) + (size_t)b0 * (size_t)N * es,
+                         params_human ? params_human + (size_t)b0 * TS_NPARAM : nullptr, 0, nullptr);
+        launches += S.stats[0];
+        ++chunks;
+    }
     S.timing = timing;
     S.cur = &S.lane[0];
+    S.stats[0] = launches;
+    S.stats[1] = chunks;
     return rc;
+}
+
+// The caller's stream continues after both internal streams.
+int join_streams() {
+    TS_CUDA(cudaEventRecord(S.lane[1].ctl_done, S.hi));
+    TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.lane[1].ctl_done, 0));
+    TS_CUDA(cudaEventRecord(S.lane[2].ctl_done, S.lo));
+    TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.lane[2].ctl_done, 0));
+    return TS_OK;
 }
 
 int corpus_issue(uint64_t batch) {  // render `batch` into its slot and record the slot's ready event on `lo`
     ts_corpus_state &C = S.corpus;
     const int slot = (int)(batch % (uint64_t)C.cfg.n_ring);
     const size_t es = fmt_bytes(C.cfg.fmt);
-    const int rc = stream_batch(C.cfg.seed, batch, C.cfg.B, C.cfg.sr, C.cfg.seconds, C.cfg.fmt,
-                                C.cfg.d_params_ring + (size_t)slot * (size_t)C.cfg.B,
-                                static_cast<char *>(C.cfg.d_audio_ring) + (size_t)slot * (size_t)C.cfg.B * (size_t)C.N * es);
+    const int rc = stream_batch(C.cfg.d_params_ring + (size_t)slot * (size_t)C.cfg.B,
+                                sample_spec{true, C.cfg.seed, batch * (uint64_t)C.cfg.B}, C.cfg.B, C.cfg.sr, C.cfg.seconds, C.cfg.fmt,
+                                static_cast<char *>(C.cfg.d_audio_ring) + (size_t)slot * (size_t)C.cfg.B * (size_t)C.N * es, nullptr);
     if (rc) return rc;
     TS_CUDA(cudaEventRecord(C.ready[slot], S.lo));
     return TS_OK;
+}
+
+// A batch that needs several voice chunks (control table capped for L2) runs its chunks on the two internal lanes, so
+// that setup + control of chunk k+1 overlap the audio kernel of chunk k; a single-chunk batch stays on the set stream.
+int render_audio(ts_voice *d_params, sample_spec smp, int B, int sr, double seconds, int fmt, void *d_audio, float *d_params_human) {
+    int64_t N;
+    int K;
+    int rc = check_sizes(B, sr, seconds, &N, &K);
+    if (rc) return rc;
+    if (chunk_voices(B, K) >= B || S.timing || S.corpus.open)
+        return render_impl(d_params, smp, B, sr, seconds, fmt, d_audio, d_params_human, 0, nullptr);
+    if (!fmt_ok(fmt)) return fail(TS_EINVAL, "unknown output format%s");
+    S.cur = &S.lane[0];
+    rc = prepare_common(sr);
+    if (rc) return rc;
+    rc = ensure_streams();
+    if (rc) return rc;
+    rc = fork_streams();
+    if (rc) return rc;
+    rc = stream_batch(d_params, smp, B, sr, seconds, fmt, d_audio, d_params_human);
+    const int rj = join_streams();
+    return rc ? rc : rj;
 }
 
 }  // namespace
@@ -407,8 +456,7 @@ int ts_sample_params(uint64_t seed, uint64_t batch_index, int B, ts_voice *d_par
 int ts_render_fmt(const ts_voice *d_params, int B, int sr, double seconds, int fmt, void *d_audio, float *d_params_human) {
     if (!d_params) return fail(TS_ENULL, "d_params is NULL%s");
     if (!d_audio) return fail(TS_ENULL, "audio is NULL%s");
-    return render_impl(const_cast<ts_voice *>(d_params), sample_spec{false, 0, 0}, B, sr, seconds, fmt, d_audio, d_params_human, 0,
-                       nullptr);
+    return render_audio(const_cast<ts_voice *>(d_params), sample_spec{false, 0, 0}, B, sr, seconds, fmt, d_audio, d_params_human);
 }
 
 int ts_render(const ts_voice *d_params, int B, int sr, double seconds, ts_out out) {
@@ -439,7 +487,7 @@ int ts_render_host_fmt(uint64_t seed, uint64_t batch_index, int B, int sr, doubl
     }
     ts_voice *d_params = static_cast<ts_voice *>(S.stage);
     void *d_audio = static_cast<char *>(S.stage) + pbytes;
-    rc = render_impl(d_params, sample_spec{true, seed, batch_index * (uint64_t)B}, B, sr, seconds, fmt, d_audio, nullptr, 0, nullptr);
+    rc = render_audio(d_params, sample_spec{true, seed, batch_index * (uint64_t)B}, B, sr, seconds, fmt, d_audio, nullptr);
     if (rc) return rc;
     TS_CUDA(cudaMemcpyAsync(host_audio, d_audio, abytes, cudaMemcpyDeviceToHost, S.cur->stream));
     if (host_params)
@@ -475,17 +523,13 @@ int ts_corpus_render_fmt(uint64_t seed, uint64_t first_batch, int n_batches, int
     int64_t launches = 0;
     for (int i = 0; i < n_batches && rc == TS_OK; ++i) {
         const size_t slot = (size_t)(i % n_ring);
-        rc = stream_batch(seed, first_batch + (uint64_t)i, B, sr, seconds, fmt, d_params_ring + slot * (size_t)B,
-                          static_cast<char *>(d_audio_ring) + slot * (size_t)B * (size_t)N * es);
+        rc = stream_batch(d_params_ring + slot * (size_t)B, sample_spec{true, seed, (first_batch + (uint64_t)i) * (uint64_t)B}, B, sr,
+                          seconds, fmt, static_cast<char *>(d_audio_ring) + slot * (size_t)B * (size_t)N * es, nullptr);
         launches += S.stats[0];
     }
-    // join: the caller's stream continues after both internal streams
-    TS_CUDA(cudaEventRecord(S.lane[1].ctl_done, S.hi));
-    TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.lane[1].ctl_done, 0));
-    TS_CUDA(cudaEventRecord(S.lane[2].ctl_done, S.lo));
-    TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.lane[2].ctl_done, 0));
+    const int rj = join_streams();
     S.stats[0] = launches;  // kernels launched by this call (3 per batch and voice chunk)
-    return rc;
+    return rc ? rc : rj;
 }
 
 int ts_corpus_render(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds,

@@ -119,6 +119,6 @@ cudaError_t ts_launch_mmd(const float *d_x, const float *d_y, int n, int d, doub
 }
 
 cudaError_t ts_launch_fill(void *d_dst, size_t bytes, cudaStream_t st) {
-    ts_fill_kernel<<<148 * 8, 256, 0, st>>>(static_cast<float4 *>(d_dst), bytes / 16);
+    ts_fill_kernel<<<148 * 32, 256, 0, st>>>(static_cast<float4 *>(d_dst), bytes / 16);
     return cudaGetLastError();
 }
