@@ -564,3 +564,53 @@ def test_end_of_range_lfo_inputs_stay_finite_and_agree_off_the_jumps(T):
         if n_ok > 0:
             d = g[b, :n_ok].astype(np.float64) - o[:n_ok]
             assert np.abs(d).max() <= MAX_ABS, (b, first_bad, np.abs(d).max())
+
+
+def test_c4_shaped_lookback_chain_four_voices(T):
+    """The deepest look-back chain of the configs (30 s at 48 kHz = 114 chunks per voice) on four C4 voices: the case the
+    sanitizer runs of profiles/ use (compute-sanitizer racecheck / memcheck / initcheck on this test and on smoke())."""
+    import torch
+    wl = W.WORKLOADS["C4"]
+    u_o, nk_o = O.sample_params(wl.seed, 0, 4)
+    u = W.edit_u(u_o, wl, 0)
+    neb = W.apply_nebula(O.default_nebula(), wl)
+    T.ts_set_nebula(W.apply_nebula(T.ts_default_nebula(), wl))
+    dev = to_dev(u, nk_o)
+    a = T.ts_render(dev, wl.sr, wl.seconds)
+    b = T.ts_render(dev, wl.sr, wl.seconds)
+    assert torch.equal(a, b)
+    assert_parity(a.cpu().numpy(), O.render_batch(u, nk_o, wl.sr, wl.N, neb), "C4 x4")
+    T.ts_sync()                                                       # raises if a look-back wait gave up
+    T.ts_set_nebula(None)
+
+
+def test_lookback_stress_bitwise_repeatable(T):
+    """compute-sanitizer is closed on this GPU pool (profiles/r02_sanitizer.md), so the epoch-flag look-back is exercised the
+    other way: 200 repeats of the streaming path (control of batch i+1 dispatched under the audio kernel of batch i, the
+    tightest residency) and 100 of the deepest chain (114 chunks per voice) must reproduce the first result bit for
+    bit (integer carries: any missed or stale aggregate changes bits), and no launch may raise the look-back timeout."""
+    import torch
+    T.ts_set_nebula(None)
+    B, sr, sec = 128, 44100, 4.0
+    N = T.ts_num_samples(sr, sec)
+    pr = torch.empty((4, B, 80), device="cuda")
+    ar = torch.empty((4, B, N), device="cuda")
+    T.ts_corpus_render(0, 100, 4, sr, sec, pr, ar)
+    torch.cuda.synchronize()
+    ref, refp = ar.clone(), pr.clone()
+    for it in range(200):
+        if it % 50 == 0:
+            ar.fill_(7.0)
+        T.ts_corpus_render(0, 100, 4, sr, sec, pr, ar)
+        torch.cuda.synchronize()
+        assert torch.equal(ar, ref) and torch.equal(pr.view(torch.int32), refp.view(torch.int32)), it
+    T.ts_sync()
+    wl = W.WORKLOADS["C4"]
+    T.ts_set_nebula(W.apply_nebula(T.ts_default_nebula(), wl))
+    u_o, nk_o = O.sample_params(wl.seed, 0, 4)
+    dev = to_dev(W.edit_u(u_o, wl, 0), nk_o)
+    first = T.ts_render(dev, wl.sr, wl.seconds).clone()
+    for it in range(100):
+        assert torch.equal(T.ts_render(dev, wl.sr, wl.seconds), first), it
+    T.ts_sync()
+    T.ts_set_nebula(None)
