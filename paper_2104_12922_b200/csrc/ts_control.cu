@@ -207,16 +207,9 @@ __device__ __forceinline__ double ts_sin2pi(double p) {
     double y = 2.0 * p - 1.0;
     y = (fabs(y) > 0.5) ? copysign(1.0, y) - y : y;
     const double y2 = y * y;
-    double q = -2.29484289972698730e-08;
-    q = fma(q, y2, 7.95205400147551261e-07);
-    q = fma(q, y2, -2.19153534478302173e-05);
-    q = fma(q, y2, 4.66302805767612554e-04);
-    q = fma(q, y2, -7.37043094571435044e-03);
-    q = fma(q, y2, 8.21458866111282326e-02);
-    q = fma(q, y2, -5.99264529320792105e-01);
-    q = fma(q, y2, 2.55016403987734552e+00);
-    q = fma(q, y2, -5.16771278004997026e+00);
-    q = fma(q, y2, 3.14159265358979312e+00);
+    double q = c_coef.sin2pip[9];
+#pragma unroll
+    for (int k = 8; k >= 0; --k) q = fma(q, y2, c_coef.sin2pip[k]);
     return -(q * y);
 }
 
@@ -242,9 +235,13 @@ ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64
                 ts_voice_consts *__restrict__ vc, ts_vhdr *__restrict__ hdr, float *__restrict__ params_human,
                 unsigned long long *__restrict__ d_active, int full) {
     __shared__ ts_voice_consts V;
+    __shared__ ts_math_tables MT;
     __shared__ __align__(16) float su[TS_NPARAM + 2];
     __shared__ uint32_t s_nk[2];
+    __shared__ float s_tanh_c;
     const int tid = threadIdx.x, v = blockIdx.x;
+    if (tid < (int)(sizeof(ts_math_tables) / 8))  // table look-ups from shared memory: ~30 cycles instead of an L2 round trip each
+        reinterpret_cast<double *>(&MT)[tid] = reinterpret_cast<const double *>(&c_math)[tid];
     if (sample) {  // S1: Philox blocks 0..19 carry the parameters, thread 20 draws the noise key (D4)
         const uint64_t g = g0 + (uint64_t)v;
         const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
@@ -271,7 +268,7 @@ ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64
         __syncthreads();
     }
     if (tid < TS_NPARAM) {
-        const double hv = ts_map((double)su[tid], c_nebula[tid], &c_math);
+        const double hv = ts_map((double)su[tid], c_nebula[tid], &MT);
         V.h[tid] = hv;
         if (params_human) params_human[(size_t)v * TS_NPARAM + tid] = (float)hv;
     }
@@ -305,6 +302,10 @@ ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64
         const double lsum = (h[75] + h[76]) + h[77];
         const double gi = (lsum == 0.0) ? 0.0 : h[75 + i] / lsum;
         V.g[i] = (i == 1) ? gi * (1.0 - h[74] / 2.0) : gi;  // VCO2 carries (1 - s/2) of S11
+    } else if (tid == 50) {  // S11: steepness of the square/saw from the unmodulated note frequency, as the tanh constant
+        const double fc = 440.0 * ts_exp2((h[0] + h[71] - 69.0) * (1.0 / 12.0), &MT);
+        const double k = 12000.0 / (fc * (ts_log2(fc, &MT) * 0.30102999566398120));
+        s_tanh_c = (float)(1.5707963267948966 * k * 2.0 * 1.4426950408889634);
     } else if (tid >= 96) {
         // The voice is silent for good once the release of all four audible envelopes is over (their
         // ramp is 1, so E = 0 exactly): adsr1, adsr2, lfo1_amp, lfo2_amp.  jsil = first tick with
@@ -324,31 +325,32 @@ ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64
             while (!silent_at(j)) ++j;
         }
         j = __shfl_sync(0xffffffffu, j, 0);
-        if (tid == 96) {  // one thread writes the results
+        if (tid == 96) {
             if (full) j = K;  // debug exports: evaluate every tick
             V.jsil = (int)j;
             int slow = 0;
             for (int e = 0; e < 6; ++e) slow |= !(h[6 + 5 * e] > 0.0);
             V.slow = slow;
             V.pad[0] = V.pad[1] = 0;
-            const long long n_act = (j * R < N) ? j * R : N;
-            ts_vhdr hd;
-            hd.shape = (float)h[74];
-            const double fc = 440.0 * ts_exp2((h[0] + h[71] - 69.0) * (1.0 / 12.0), &c_math);
-            const double k = 12000.0 / (fc * (ts_log2(fc, &c_math) * 0.30102999566398120));
-            hd.tanh_c = (float)(1.5707963267948966 * k * 2.0 * 1.4426950408889634);
-            hd.nk0 = s_nk[0];
-            hd.nk1 = s_nk[1];
-            hd.n_act = (int32_t)n_act;
-            hd.n_ticks = (int32_t)((j + 1 < K) ? j + 1 : K);
-            hd.pad[0] = hd.pad[1] = 0;
-            hdr[v] = hd;
-            if (d_active) atomicAdd(d_active, (unsigned long long)n_act);
         }
     }
     __syncthreads();
     if (tid < (int)(sizeof(ts_voice_consts) / 16))
         reinterpret_cast<uint4 *>(vc + v)[tid] = reinterpret_cast<const uint4 *>(&V)[tid];
+    if (tid == 96) {  // the voice header of the audio kernel
+        const long long j = V.jsil;
+        const long long n_act = (j * R < N) ? j * R : N;
+        ts_vhdr hd;
+        hd.shape = (float)h[74];
+        hd.tanh_c = s_tanh_c;
+        hd.nk0 = s_nk[0];
+        hd.nk1 = s_nk[1];
+        hd.n_act = (int32_t)n_act;
+        hd.n_ticks = (int32_t)((j + 1 < K) ? j + 1 : K);
+        hd.pad[0] = hd.pad[1] = 0;
+        hdr[v] = hd;
+        if (d_active) atomicAdd(d_active, (unsigned long long)n_act);
+    }
 }
 
 // PHASES = 1: controls + the S9 tick-level phase scan + the control table of the audio kernel;

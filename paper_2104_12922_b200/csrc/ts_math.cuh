@@ -18,6 +18,25 @@ struct ts_math_tables {
 };
 
 #ifdef __CUDACC__
+// Polynomial coefficients live in constant memory: an fp64 instruction takes a constant-bank operand directly, whereas a
+// double literal in the code costs two extra moves per coefficient (the two 32-bit halves) in front of every DFMA.
+struct ts_math_coefs {
+    double log2p[10];   // log2(1+r) = r * sum_k log2p[k] r^k, log2p[k] = (-1)^k log2(e) / (k + 1)
+    double exp2p[6];    // 2^f - 1 = f * sum_k exp2p[k] f^k, exp2p[k] = ln2^(k+1) / (k+1)!
+    double expm1p[11];  // expm1(a) = a + a^2 * sum_k expm1p[k] a^k, expm1p[k] = 1 / (k+2)!
+    double sin2pip[10]; // sin(pi y) = y * sum_k sin2pip[k] y^(2k)
+};
+__constant__ ts_math_coefs c_coef = {
+    {1.4426950408889634, -1.4426950408889634 / 2.0, 1.4426950408889634 / 3.0, -1.4426950408889634 / 4.0, 1.4426950408889634 / 5.0,
+     -1.4426950408889634 / 6.0, 1.4426950408889634 / 7.0, -1.4426950408889634 / 8.0, 1.4426950408889634 / 9.0, 0.0},
+    {0.6931471805599453, 0.6931471805599453 * 0.6931471805599453 / 2.0, 0.6931471805599453 * 0.6931471805599453 * 0.6931471805599453 / 6.0,
+     0.6931471805599453 * 0.6931471805599453 * 0.6931471805599453 * 0.6931471805599453 / 24.0,
+     0.6931471805599453 * 0.6931471805599453 * 0.6931471805599453 * 0.6931471805599453 * 0.6931471805599453 / 120.0,
+     0.6931471805599453 * 0.6931471805599453 * 0.6931471805599453 * 0.6931471805599453 * 0.6931471805599453 * 0.6931471805599453 / 720.0},
+    {0.5, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0, 1.0 / 5040.0, 1.0 / 40320.0, 1.0 / 362880.0, 1.0 / 3628800.0,
+     1.0 / 39916800.0, 1.0 / 479001600.0},
+    {3.14159265358979312e+00, -5.16771278004997026e+00, 2.55016403987734552e+00, -5.99264529320792105e-01, 8.21458866111282326e-02,
+     -7.37043094571435044e-03, 4.66302805767612554e-04, -2.19153534478302173e-05, 7.95205400147551261e-07, -2.29484289972698730e-08}};
 // log2(x), x > 0 normal.  x = 2^k z, z in [0.6875, 1.375); r = z*invc - 1 (|r| < 0.0157, exact in an FMA up to
 // 2^-59); log2 x = k + logc + log2(1+r).
 __device__ __forceinline__ double ts_log2(double x, const ts_math_tables *T) {
@@ -28,15 +47,9 @@ __device__ __forceinline__ double ts_log2(double x, const ts_math_tables *T) {
     const double z = __longlong_as_double((long long)(ix - (tmp & 0xFFF0000000000000ull)));
     const double r = fma(z, T->invc[i], -1.0);
     // log2(1+r) = r * log2(e) * (1 - r/2 + r^2/3 - ...), degree 9 in r
-    double p = 1.4426950408889634 / 9.0;
-    p = fma(p, r, -1.4426950408889634 / 8.0);
-    p = fma(p, r, 1.4426950408889634 / 7.0);
-    p = fma(p, r, -1.4426950408889634 / 6.0);
-    p = fma(p, r, 1.4426950408889634 / 5.0);
-    p = fma(p, r, -1.4426950408889634 / 4.0);
-    p = fma(p, r, 1.4426950408889634 / 3.0);
-    p = fma(p, r, -1.4426950408889634 / 2.0);
-    p = fma(p, r, 1.4426950408889634);
+    double p = c_coef.log2p[8];
+#pragma unroll
+    for (int k = 7; k >= 0; --k) p = fma(p, r, c_coef.log2p[k]);
     return fma(p, r, (double)k + T->logc[i]);
 }
 
@@ -47,13 +60,9 @@ __device__ __forceinline__ double ts_exp2(double y, const ts_math_tables *T) {
     const int n = __double2loint(kd);        // rint(32 y)
     const double f = fma(kd - big, -1.0 / 32.0, y);
     // 2^f = exp(f ln2), degree 6
-    const double L = 0.6931471805599453;
-    double p = L * L * L * L * L * L / 720.0;
-    p = fma(p, f, L * L * L * L * L / 120.0);
-    p = fma(p, f, L * L * L * L / 24.0);
-    p = fma(p, f, L * L * L / 6.0);
-    p = fma(p, f, L * L / 2.0);
-    p = fma(p, f, L);
+    double p = c_coef.exp2p[5];
+#pragma unroll
+    for (int k = 4; k >= 0; --k) p = fma(p, f, c_coef.exp2p[k]);
     const double t = T->exp2t[n & (TS_EXP_N - 1)];
     const double v = fma(t * p, f, t);
     const int e = n >> 5;
@@ -70,17 +79,9 @@ __device__ __forceinline__ double ts_pow01(double x, double a, const ts_math_tab
 // expm1(a) for |a| <= 0.125 by its series (relative accuracy down to a -> 0); libdevice beyond.
 __device__ __forceinline__ double ts_expm1_small(double a) {
     if (fabs(a) > 0.125) return expm1(a);
-    double p = 1.0 / 479001600.0;          // 1/12!
-    p = fma(p, a, 1.0 / 39916800.0);
-    p = fma(p, a, 1.0 / 3628800.0);
-    p = fma(p, a, 1.0 / 362880.0);
-    p = fma(p, a, 1.0 / 40320.0);
-    p = fma(p, a, 1.0 / 5040.0);
-    p = fma(p, a, 1.0 / 720.0);
-    p = fma(p, a, 1.0 / 120.0);
-    p = fma(p, a, 1.0 / 24.0);
-    p = fma(p, a, 1.0 / 6.0);
-    p = fma(p, a, 0.5);
+    double p = c_coef.expm1p[10];          // 1/12!
+#pragma unroll
+    for (int k = 9; k >= 0; --k) p = fma(p, a, c_coef.expm1p[k]);
     return fma(p * a, a, a);
 }
 #endif
