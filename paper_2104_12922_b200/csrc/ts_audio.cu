@@ -86,14 +86,16 @@ constexpr float SIN_C3 = -0.16666659712791443f, SIN_C5 = 0.008333087898790836f, 
 template <int MODE, int TAIL, int FMT>
 __global__ void __launch_bounds__(TS_AUDIO_THREADS)
 ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ hdr, int B, long long N, int K,
-                void *__restrict__ audio_, double *__restrict__ dbg_phase, int aligned, uint32_t one_bits) {
+                void *__restrict__ audio_, double *__restrict__ dbg_phase, int aligned, uint32_t one_bits, int swap) {
     __shared__ __align__(128) float4 stage[TS_TILE / 4];
     __shared__ __align__(128) float4 zero[(MODE == 0 && TAIL) ? TS_TILE / 4 : 4];  // source of the tail's zero-fill bulk copies
 
     constexpr int ES = (FMT == TS_F32) ? 4 : 2;  // bytes per output sample
     char *audio = static_cast<char *>(audio_);
-    const int voice = blockIdx.x % B;  // time-major grid: the audible (expensive) tiles are dispatched first
-    const long long tile = blockIdx.x / B;
+    // 2-D grid, no integer division: x = voice, y = tile (x runs fastest: time-major dispatch, the audible tiles of all
+    // voices go first); swapped when a voice has more than 65535 tiles
+    const int voice = swap ? blockIdx.y : blockIdx.x;
+    const long long tile = swap ? blockIdx.x : blockIdx.y;
     const long long n_tile0 = tile * TS_TILE;
     const int tid = threadIdx.x;
     const ts_vhdr hd = hdr[voice];
@@ -282,14 +284,14 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
 cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, void *audio, int fmt,
                             int mode, int tails, double *dbg_phase, cudaStream_t st) {
     const int64_t tiles = (N + TS_TILE - 1) / TS_TILE;
-    const int64_t grid = tiles * B;
-    if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
+    if (tiles > 0x7fffffffLL || (tiles > 65535 && B > 65535)) return cudaErrorInvalidValue;
+    const int swap = tiles > 65535;
+    const dim3 g = swap ? dim3((unsigned)tiles, (unsigned)B) : dim3((unsigned)B, (unsigned)tiles);
     // bulk copies and 128-bit stores need 16-byte aligned rows: N a multiple of 4 (fp32) or 8 (16-bit) samples
     const int per16 = (fmt == TS_F32) ? 4 : 8;
     const int aligned = (N % per16 == 0) && ((reinterpret_cast<uintptr_t>(audio) & 15u) == 0);
-    const unsigned g = (unsigned)grid;
 #define TS_LAUNCH(MODE, TAIL, FMT) \
-    ts_audio_kernel<MODE, TAIL, FMT><<<g, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u)
+    ts_audio_kernel<MODE, TAIL, FMT><<<g, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u, swap)
     if (mode == 0) {
         if (fmt == TS_F32) { if (tails) TS_LAUNCH(0, 1, TS_F32); else TS_LAUNCH(0, 0, TS_F32); }
         else if (fmt == TS_F16) { if (tails) TS_LAUNCH(0, 1, TS_F16); else TS_LAUNCH(0, 0, TS_F16); }

@@ -359,7 +359,7 @@ template <int PHASES>
 __global__ void __launch_bounds__(TS_CTL_THREADS)
 ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, long long N, int K, int NC,
                   ts_tick *__restrict__ table, ts_agg *__restrict__ agg, unsigned int epoch, double *__restrict__ dbg_ctl,
-                  unsigned int *__restrict__ err) {
+                  unsigned int *__restrict__ err, int swap) {
     __shared__ ts_voice_consts V;
     __shared__ ts_math_tables MT;
     __shared__ unsigned long long scan_sm[64];
@@ -368,7 +368,9 @@ ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, 
     __shared__ double Es[6][TS_CTL_THREADS];
 
     const int tid = threadIdx.x;
-    const int c = blockIdx.x / B, v = blockIdx.x - c * B;  // chunk-major: predecessors have lower block indices
+    // 2-D grid, no integer division (x = voice, y = chunk; swapped when a voice has more than 65535 chunks): either way
+    // a chunk's predecessors have lower linear block indices
+    const int c = swap ? blockIdx.x : blockIdx.y, v = swap ? blockIdx.y : blockIdx.x;
     const int j0 = c * TS_CTL_IC;
     const int jsil = vc[v].jsil;
     if (c > 0 && j0 >= jsil) {  // nothing audible from this chunk on (55 % of C2's chunks); no successor waits for it
@@ -513,14 +515,15 @@ cudaError_t ts_launch_control(const ts_voice_consts *vc, int B, int sr, int R, i
     const int J = K - 1;
     int NC = (J + TS_CTL_IC - 1) / TS_CTL_IC;
     if (NC < 1) NC = 1;
-    const long long grid = (long long)NC * B;
-    if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
+    if (NC > 65535 && B > 65535) return cudaErrorInvalidValue;
+    const int swap = NC > 65535;
+    const dim3 grid = swap ? dim3((unsigned)NC, (unsigned)B) : dim3((unsigned)B, (unsigned)NC);
     if (phases && R != TS_R) return cudaErrorInvalidValue;  // the audio kernel's geometry is built on R = 100
     if (phases)
-        ts_control_kernel<1><<<(unsigned)grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
-                                                                       static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err);
+        ts_control_kernel<1><<<grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
+                                                                       static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err, swap);
     else
-        ts_control_kernel<0><<<(unsigned)grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
-                                                                       static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err);
+        ts_control_kernel<0><<<grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
+                                                                       static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err, swap);
     return cudaGetLastError();
 }
