@@ -79,6 +79,77 @@ template <int FMT> __device__ __forceinline__ uint32_t ts_cvt16(ts_f2 v) {
 // has slope up to ~1e5 per cycle at the zero crossings, H4).
 constexpr float SIN_C3 = -0.16666659712791443f, SIN_C5 = 0.008333087898790836f, SIN_C7 = -0.00019811101083178073f,
                 SIN_C9 = 2.6089039693033556e-06f;
+// The 20 samples of one run (S9..S14) from its start state, into the thread's slice of the staging tile.
+// FASTSIN: the square/saw's sine through MUFU.SIN (absolute error 2^-21: 3.7e-7) instead of the relative-accuracy
+// polynomial.  The sine is multiplied by (pi/2) k before the tanh (S11), so this is only taken for voices whose
+// steepness k <= 256 (four voices in five under the default nebula): the error it adds to a sample is then below
+// (pi/2) 256 * 3.7e-7 * 1.125 = 1.7e-4, a tenth of the 2e-3 bar (H4; the flag is set by the setup kernel).
+template <int FMT, int FASTSIN>
+__device__ __forceinline__ void ts_render_run(double P1, double w1, const double e1a, double P2, double w2, const double e1b,
+                                              float a1, float a2, float a3, const float da1, const float da2, const float da3,
+                                              const uint32_t blk0, const uint32_t nk0, const uint32_t nk1, const float shape,
+                                              const float tanh_c, const uint32_t one_bits, float4 *my, uint2 *my16) {
+        const ts_f2 SHAPE = ts_dup(shape), TANH_C = ts_dup(tanh_c), ONE = ts_dup(1.0f);
+        ts_f2 G1 = ts_pack(a1, a1 + da1), G2 = ts_pack(a2, a2 + da2), G3 = ts_pack(a3, a3 + da3);
+        const ts_f2 DG1 = ts_dup(2.0f * da1), DG2 = ts_dup(2.0f * da2), DG3 = ts_dup(2.0f * da3);
+        ulonglong2 *my2 = reinterpret_cast<ulonglong2 *>(my);
+#pragma unroll
+        for (int g = 0; g < TS_RUN / 4; ++g) {
+            uint32_t nz[4];
+            ts_philox4x32_10(blk0 + g, 0u, 0u, 1u, nk0, nk1, nz);  // S12
+            ts_f2 O[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                // ---- S9: phase accumulation for two consecutive samples (fp64, geometric increments)
+                const int xa = __double2loint(P1);
+                const int la = __double2loint(P2), ha = __double2hiint(P2);
+                P1 += w1; w1 = fma(w1, e1a, w1);
+                P2 += w2; w2 = fma(w2, e1b, w2);
+                const int xb = __double2loint(P1);
+                const int lb = __double2loint(P2), hb = __double2hiint(P2);
+                P1 += w1; w1 = fma(w1, e1a, w1);
+                P2 += w2; w2 = fma(w2, e1b, w2);
+                // ---- S10 sine VCO: frac(phi) is the signed Q0.32 in the low word
+                float r1a, r1b;
+                ts_unpack(ts_mul2(ts_pack((float)xa, (float)xb), ts_dup(1.4629180792671596e-9f)), r1a, r1b);  // 2 pi 2^-32
+                const ts_f2 Y1 = ts_pack(__sinf(r1a), __sinf(r1b));
+                // ---- S11 square/saw VCO: low word = signed Q0.32 of the nearest HALF cycle (H4); the parity of
+                // that half cycle (bit 0 of the high word, +1 if the low word is negative) is the sign sigma.
+                const uint32_t sa = (((uint32_t)la + ((uint32_t)ha << 31)) & 0x80000000u) | one_bits;
+                const uint32_t sb = (((uint32_t)lb + ((uint32_t)hb << 31)) & 0x80000000u) | one_bits;
+                const ts_f2 SIG = ts_pack(__uint_as_float(sa), __uint_as_float(sb));
+                const ts_f2 TH = ts_mul2(ts_pack((float)la, (float)lb), ts_dup(7.314590396335798e-10f));  // 2 pi 2^-33
+                float ea, eb, da, db;
+                float tha, thb;
+                ts_unpack(TH, tha, thb);
+                ts_f2 SN;  // sin(th), th in [-pi/2, pi/2)
+                if (FASTSIN) {
+                    SN = ts_pack(__sinf(tha), __sinf(thb));
+                } else {
+                    const ts_f2 T2 = ts_mul2(TH, TH);
+                    ts_f2 Q = ts_fma2(T2, ts_dup(SIN_C9), ts_dup(SIN_C7));
+                    Q = ts_fma2(Q, T2, ts_dup(SIN_C5));
+                    Q = ts_fma2(Q, T2, ts_dup(SIN_C3));
+                    SN = ts_fma2(ts_mul2(TH, T2), Q, TH);
+                }
+                const ts_f2 CS = ts_pack(__cosf(tha), __cosf(thb));
+                ts_unpack(ts_mul2(SN, TANH_C), ea, eb);
+                ts_unpack(ts_add2(ts_pack(ts_ex2(ea), ts_ex2(eb)), ONE), da, db);
+                // tanh((pi/2) k sin) = 1 - 2 / (1 + 2^(c sin));  y2 = sigma tanh (1 + s sigma cos) = tanh (sigma + s cos)
+                const ts_f2 TNH = ts_fma2(ts_pack(ts_rcp(da), ts_rcp(db)), ts_dup(-2.0f), ONE);
+                const ts_f2 Y2 = ts_mul2(TNH, ts_fma2(SHAPE, CS, SIG));
+                // ---- S12 noise value (RZ conversion keeps the top 24 bits of x when x >= 2^31 and a few more
+                // below: within 2^-24 of (x >> 8) 2^-23 - 1), S13 VCAs, S14 mixer (gains carry the mixer levels)
+                const ts_f2 Z = ts_fma2(ts_pack(__uint2float_rz(nz[2 * h]), __uint2float_rz(nz[2 * h + 1])),
+                                        ts_dup(4.656612873077393e-10f), ts_dup(-1.0f));
+                O[h] = ts_fma2(G3, Z, ts_fma2(G2, Y2, ts_mul2(G1, Y1)));
+                G1 = ts_add2(G1, DG1); G2 = ts_add2(G2, DG2); G3 = ts_add2(G3, DG3);
+            }
+            if (FMT == TS_F32) my2[g] = make_ulonglong2(O[0], O[1]);
+            else my16[g] = make_uint2(ts_cvt16<FMT>(O[0]), ts_cvt16<FMT>(O[1]));
+        }
+}
+
 // TAIL = 1: the silent tails are written by the audible CTAs (below); TAIL = 0: every silent tile is written by a CTA of
 // its own (better when few tiles are silent: no zero buffer, more L1 left for the control table).
 // FMT: output sample format (TS_F32 / TS_F16 / TS_BF16): the finished fp32 sample is rounded once, two samples per
@@ -190,60 +261,12 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
         double P1 = p1 + MAGIC32, P2 = p2 + MAGIC33;
 
         if (MODE == 0) {
-            const ts_f2 SHAPE = ts_dup(hd.shape), TANH_C = ts_dup(hd.tanh_c), ONE = ts_dup(1.0f);
-            ts_f2 G1 = ts_pack(a1, a1 + da1), G2 = ts_pack(a2, a2 + da2), G3 = ts_pack(a3, a3 + da3);
-            const ts_f2 DG1 = ts_dup(2.0f * da1), DG2 = ts_dup(2.0f * da2), DG3 = ts_dup(2.0f * da3);
-            ulonglong2 *my2 = reinterpret_cast<ulonglong2 *>(my);
-#pragma unroll
-            for (int g = 0; g < TS_RUN / 4; ++g) {
-                uint32_t nz[4];
-                ts_philox4x32_10(blk0 + g, 0u, 0u, 1u, hd.nk0, hd.nk1, nz);  // S12
-                ts_f2 O[2];
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    // ---- S9: phase accumulation for two consecutive samples (fp64, geometric increments)
-                    const int xa = __double2loint(P1);
-                    const int la = __double2loint(P2), ha = __double2hiint(P2);
-                    P1 += w1; w1 = fma(w1, e1a, w1);
-                    P2 += w2; w2 = fma(w2, e1b, w2);
-                    const int xb = __double2loint(P1);
-                    const int lb = __double2loint(P2), hb = __double2hiint(P2);
-                    P1 += w1; w1 = fma(w1, e1a, w1);
-                    P2 += w2; w2 = fma(w2, e1b, w2);
-                    // ---- S10 sine VCO: frac(phi) is the signed Q0.32 in the low word
-                    float r1a, r1b;
-                    ts_unpack(ts_mul2(ts_pack((float)xa, (float)xb), ts_dup(1.4629180792671596e-9f)), r1a, r1b);  // 2 pi 2^-32
-                    const ts_f2 Y1 = ts_pack(__sinf(r1a), __sinf(r1b));
-                    // ---- S11 square/saw VCO: low word = signed Q0.32 of the nearest HALF cycle (H4); the parity of
-                    // that half cycle (bit 0 of the high word, +1 if the low word is negative) is the sign sigma.
-                    const uint32_t sa = (((uint32_t)la + ((uint32_t)ha << 31)) & 0x80000000u) | one_bits;
-                    const uint32_t sb = (((uint32_t)lb + ((uint32_t)hb << 31)) & 0x80000000u) | one_bits;
-                    const ts_f2 SIG = ts_pack(__uint_as_float(sa), __uint_as_float(sb));
-                    const ts_f2 TH = ts_mul2(ts_pack((float)la, (float)lb), ts_dup(7.314590396335798e-10f));  // 2 pi 2^-33
-                    const ts_f2 T2 = ts_mul2(TH, TH);
-                    ts_f2 Q = ts_fma2(T2, ts_dup(SIN_C9), ts_dup(SIN_C7));
-                    Q = ts_fma2(Q, T2, ts_dup(SIN_C5));
-                    Q = ts_fma2(Q, T2, ts_dup(SIN_C3));
-                    const ts_f2 SN = ts_fma2(ts_mul2(TH, T2), Q, TH);  // sin(th), th in [-pi/2, pi/2)
-                    float ea, eb, da, db;
-                    float tha, thb;
-                    ts_unpack(TH, tha, thb);
-                    const ts_f2 CS = ts_pack(__cosf(tha), __cosf(thb));
-                    ts_unpack(ts_mul2(SN, TANH_C), ea, eb);
-                    ts_unpack(ts_add2(ts_pack(ts_ex2(ea), ts_ex2(eb)), ONE), da, db);
-                    // tanh((pi/2) k sin) = 1 - 2 / (1 + 2^(c sin));  y2 = sigma tanh (1 + s sigma cos) = tanh (sigma + s cos)
-                    const ts_f2 TNH = ts_fma2(ts_pack(ts_rcp(da), ts_rcp(db)), ts_dup(-2.0f), ONE);
-                    const ts_f2 Y2 = ts_mul2(TNH, ts_fma2(SHAPE, CS, SIG));
-                    // ---- S12 noise value (RZ conversion keeps the top 24 bits of x when x >= 2^31 and a few more
-                    // below: within 2^-24 of (x >> 8) 2^-23 - 1), S13 VCAs, S14 mixer (gains carry the mixer levels)
-                    const ts_f2 Z = ts_fma2(ts_pack(__uint2float_rz(nz[2 * h]), __uint2float_rz(nz[2 * h + 1])),
-                                            ts_dup(4.656612873077393e-10f), ts_dup(-1.0f));
-                    O[h] = ts_fma2(G3, Z, ts_fma2(G2, Y2, ts_mul2(G1, Y1)));
-                    G1 = ts_add2(G1, DG1); G2 = ts_add2(G2, DG2); G3 = ts_add2(G3, DG3);
-                }
-                if (FMT == TS_F32) my2[g] = make_ulonglong2(O[0], O[1]);
-                else my16[g] = make_uint2(ts_cvt16<FMT>(O[0]), ts_cvt16<FMT>(O[1]));
-            }
+            if (hd.pad[0])  // CTA-uniform: the voice's square/saw is gentle enough for MUFU.SIN
+                ts_render_run<FMT, 1>(P1, w1, e1a, P2, w2, e1b, a1, a2, a3, da1, da2, da3, blk0, hd.nk0, hd.nk1, hd.shape, hd.tanh_c,
+                                      one_bits, my, my16);
+            else
+                ts_render_run<FMT, 0>(P1, w1, e1a, P2, w2, e1b, a1, a2, a3, da1, da2, da3, blk0, hd.nk0, hd.nk1, hd.shape, hd.tanh_c,
+                                      one_bits, my, my16);
         } else {
             for (int i = 0; i < TS_RUN; ++i) {
                 const long long n = n0 + i;

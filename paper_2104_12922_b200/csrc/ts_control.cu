@@ -239,6 +239,7 @@ ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64
     __shared__ __align__(16) float su[TS_NPARAM + 2];
     __shared__ uint32_t s_nk[2];
     __shared__ float s_tanh_c;
+    __shared__ int s_fast;
     const int tid = threadIdx.x, v = blockIdx.x;
     if (tid < (int)(sizeof(ts_math_tables) / 8))  // table look-ups from shared memory: ~30 cycles instead of an L2 round trip each
         reinterpret_cast<double *>(&MT)[tid] = reinterpret_cast<const double *>(&c_math)[tid];
@@ -306,6 +307,7 @@ ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64
         const double fc = 440.0 * ts_exp2((h[0] + h[71] - 69.0) * (1.0 / 12.0), &MT);
         const double k = 12000.0 / (fc * (ts_log2(fc, &MT) * 0.30102999566398120));
         s_tanh_c = (float)(1.5707963267948966 * k * 2.0 * 1.4426950408889634);
+        s_fast = (k <= 256.0) ? 1 : 0;
     } else if (tid >= 96) {
         // The voice is silent for good once the release of all four audible envelopes is over (their
         // ramp is 1, so E = 0 exactly): adsr1, adsr2, lfo1_amp, lfo2_amp.  jsil = first tick with
@@ -347,7 +349,8 @@ ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64
         hd.nk1 = s_nk[1];
         hd.n_act = (int32_t)n_act;
         hd.n_ticks = (int32_t)((j + 1 < K) ? j + 1 : K);
-        hd.pad[0] = hd.pad[1] = 0;
+        hd.pad[0] = s_fast;
+        hd.pad[1] = 0;
         hdr[v] = hd;
         if (d_active) atomicAdd(d_active, (unsigned long long)n_act);
     }
