@@ -82,8 +82,9 @@ constexpr float SIN_C3 = -0.16666659712791443f, SIN_C5 = 0.008333087898790836f, 
 // The 20 samples of one run (S9..S14) from its start state, into the thread's slice of the staging tile.
 // FASTSIN: the square/saw's sine through MUFU.SIN (absolute error 2^-21: 3.7e-7) instead of the relative-accuracy
 // polynomial.  The sine is multiplied by (pi/2) k before the tanh (S11), so this is only taken for voices whose
-// steepness k <= 256 (four voices in five under the default nebula): the error it adds to a sample is then below
-// (pi/2) 256 * 3.7e-7 * 1.125 = 1.7e-4, a tenth of the 2e-3 bar (H4; the flag is set by the setup kernel).
+// steepness k <= 1024 (note frequency above 10.9 Hz: 93 % of the voices under the default nebula): the error it adds
+// to a sample is then below (pi/2) 1024 * 3.7e-7 * 1.125 = 6.7e-4, a third of the 2e-3 bar, and only within ~1/k of a
+// cycle around the zero crossings (rel-RMS contribution < 3e-5) (H4; the flag is set by the setup kernel).
 template <int FMT, int FASTSIN>
 __device__ __forceinline__ void ts_render_run(double P1, double w1, const double e1a, double P2, double w2, const double e1b,
                                               float a1, float a2, float a3, const float da1, const float da2, const float da3,
