@@ -155,7 +155,9 @@ __device__ __forceinline__ void ts_render_run(double P1, double w1, const double
 // its own (better when few tiles are silent: no zero buffer, more L1 left for the control table).
 // FMT: output sample format (TS_F32 / TS_F16 / TS_BF16): the finished fp32 sample is rounded once, two samples per
 // cvt.rn.{f16x2,bf16x2}.f32, on its way into the staging tile.
-template <int MODE, int TAIL, int FMT>
+// TPC: consecutive tiles of one voice rendered by one CTA, one after the other (large launches: halves the CTA turnover,
+// which costs ~14 % of an SM's time at one tile per CTA; small launches keep TPC = 1 so that the last wave stays short).
+template <int MODE, int TAIL, int FMT, int TPC>
 __global__ void __launch_bounds__(TS_AUDIO_THREADS)
 ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ hdr, int B, long long N, int K,
                 void *__restrict__ audio_, double *__restrict__ dbg_phase, int aligned, uint32_t one_bits, int swap) {
@@ -167,10 +169,17 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
     // 2-D grid, no integer division: x = voice, y = tile (x runs fastest: time-major dispatch, the audible tiles of all
     // voices go first); swapped when a voice has more than 65535 tiles
     const int voice = swap ? blockIdx.y : blockIdx.x;
-    const long long tile = swap ? blockIdx.x : blockIdx.y;
-    const long long n_tile0 = tile * TS_TILE;
+    const long long tile_first = (swap ? blockIdx.x : blockIdx.y) * (long long)TPC;
     const int tid = threadIdx.x;
     const ts_vhdr hd = hdr[voice];
+    const long long T = (N + TS_TILE - 1) / TS_TILE;
+    bool zeroed = false;  // the zero buffer is filled once per CTA
+#pragma unroll 1
+    for (int tt = 0; tt < TPC; ++tt) {
+    const long long tile = tile_first + tt;
+    if (tile >= T) return;
+    if (TPC > 1 && tt > 0) __syncthreads();  // the previous tile's bulk copy has read the staging tile (thread 0 waited)
+    const long long n_tile0 = tile * TS_TILE;
     const long long rem = N - n_tile0;
     const int count = (rem < TS_TILE) ? (int)rem : TS_TILE;  // samples of this tile inside the buffer
     char *row = audio + ((size_t)voice * N + n_tile0) * ES;
@@ -184,25 +193,27 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
         } else {
             for (int i = tid; i < count; i += TS_AUDIO_THREADS) reinterpret_cast<unsigned short *>(row)[i] = 0;
         }
-        return;
+        continue;
     }
     if (MODE == 0 && TAIL) {
         // Samples [n_act, N) are exactly 0 (S4 release over; pin P9).  The silent tiles of a voice are not rendered by
         // CTAs of their own: audible tile t of a voice with A audible tiles writes the silent tiles A + t, A + t + A, ...
         // as asynchronous bulk copies of a zero buffer (TMA engine), issued BEFORE its arithmetic, so that the stores
         // of the tails overlap the issue-bound arithmetic of the audible part instead of following it.
-        const long long T = (N + TS_TILE - 1) / TS_TILE;
         long long A = ((long long)hd.n_act + TS_TILE - 1) / TS_TILE;
         if (A < 1) A = 1;  // a voice with no audible sample: tile 0 renders zeros and owns the whole tail
-        if (tile >= A) return;
+        if (tile >= A) return;  // and so are all later tiles of this voice
         char *vrow = audio + (size_t)voice * N * ES;
         if (A + tile >= T) {
             // no silent tile falls to this CTA
         } else if (aligned) {
+            if (!zeroed) {
 #pragma unroll
-            for (int g = 0; g < TS_RUN / 4; ++g) zero[tid * (TS_RUN / 4) + g] = make_float4(0.f, 0.f, 0.f, 0.f);
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> async proxy
-            __syncthreads();
+                for (int g = 0; g < TS_RUN / 4; ++g) zero[tid * (TS_RUN / 4) + g] = make_float4(0.f, 0.f, 0.f, 0.f);
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> async proxy
+                __syncthreads();
+                zeroed = true;
+            }
             if ((tid & 31) == 0) {  // lane 0 of each warp issues every fourth copy
                 const uint32_t zs = (uint32_t)__cvta_generic_to_shared(zero);
                 for (long long tz = A + tile + (tid >> 5) * A; tz < T; tz += (TS_AUDIO_THREADS / 32) * A) {
@@ -284,7 +295,7 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
             else my16[g] = make_uint2(0u, 0u);
         }
     }
-    if (MODE != 0) return;
+    if (MODE != 0) continue;
 
     if (aligned) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> async proxy
@@ -301,6 +312,7 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
             for (int i = tid; i < count; i += TS_AUDIO_THREADS) reinterpret_cast<unsigned short *>(row)[i] = sh[i];
         }
     }
+    }  // tiles of this CTA
 }
 
 }  // namespace
@@ -308,24 +320,29 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
 cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, void *audio, int fmt,
                             int mode, int tails, double *dbg_phase, cudaStream_t st) {
     const int64_t tiles = (N + TS_TILE - 1) / TS_TILE;
-    if (tiles > 0x7fffffffLL || (tiles > 65535 && B > 65535)) return cudaErrorInvalidValue;
-    const int swap = tiles > 65535;
-    const dim3 g = swap ? dim3((unsigned)tiles, (unsigned)B) : dim3((unsigned)B, (unsigned)tiles);
+    // two tiles per CTA once the launch is large enough to fill the GPU many times over
+    const int tpc = (mode == 0 && tiles * B >= 12000) ? 2 : 1;
+    const int64_t ty = (tiles + tpc - 1) / tpc;
+    if (ty > 0x7fffffffLL || (ty > 65535 && B > 65535)) return cudaErrorInvalidValue;
+    const int swap = ty > 65535;
+    const dim3 g = swap ? dim3((unsigned)ty, (unsigned)B) : dim3((unsigned)B, (unsigned)ty);
     // bulk copies and 128-bit stores need 16-byte aligned rows: N a multiple of 4 (fp32) or 8 (16-bit) samples
     const int per16 = (fmt == TS_F32) ? 4 : 8;
     const int aligned = (N % per16 == 0) && ((reinterpret_cast<uintptr_t>(audio) & 15u) == 0);
-#define TS_LAUNCH(MODE, TAIL, FMT) \
-    ts_audio_kernel<MODE, TAIL, FMT><<<g, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u, swap)
+#define TS_LAUNCH(MODE, TAIL, FMT, TPC) \
+    ts_audio_kernel<MODE, TAIL, FMT, TPC><<<g, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u, swap)
+#define TS_LAUNCH_T(TAIL, FMT) do { if (tpc == 2) TS_LAUNCH(0, TAIL, FMT, 2); else TS_LAUNCH(0, TAIL, FMT, 1); } while (0)
     if (mode == 0) {
-        if (fmt == TS_F32) { if (tails) TS_LAUNCH(0, 1, TS_F32); else TS_LAUNCH(0, 0, TS_F32); }
-        else if (fmt == TS_F16) { if (tails) TS_LAUNCH(0, 1, TS_F16); else TS_LAUNCH(0, 0, TS_F16); }
-        else if (fmt == TS_BF16) { if (tails) TS_LAUNCH(0, 1, TS_BF16); else TS_LAUNCH(0, 0, TS_BF16); }
+        if (fmt == TS_F32) { if (tails) TS_LAUNCH_T(1, TS_F32); else TS_LAUNCH_T(0, TS_F32); }
+        else if (fmt == TS_F16) { if (tails) TS_LAUNCH_T(1, TS_F16); else TS_LAUNCH_T(0, TS_F16); }
+        else if (fmt == TS_BF16) { if (tails) TS_LAUNCH_T(1, TS_BF16); else TS_LAUNCH_T(0, TS_BF16); }
         else return cudaErrorInvalidValue;
     } else if (mode == 1) {
-        TS_LAUNCH(1, 0, TS_F32);
+        TS_LAUNCH(1, 0, TS_F32, 1);
     } else {
-        TS_LAUNCH(2, 0, TS_F32);
+        TS_LAUNCH(2, 0, TS_F32, 1);
     }
+#undef TS_LAUNCH_T
 #undef TS_LAUNCH
     return cudaGetLastError();
 }
