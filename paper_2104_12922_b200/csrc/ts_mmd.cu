@@ -15,6 +15,7 @@ namespace {
 constexpr int MT = 64;   // pairs per tile side
 constexpr int MK = 32;   // components per shared-memory chunk
 constexpr int MTHREADS = 256;
+constexpr int MSPLIT = 4;  // CTAs per tile, each over a quarter of the components: 2112 CTAs at n = 1000 (4.8 waves)
 
 // tile list: [0, T*T) X-Y tiles (ti, tj); then T(T+1)/2 X-X tiles with tj >= ti; then as many Y-Y tiles
 __device__ __forceinline__ void ts_mmd_tile(int t, int T, int &m, int &ti, int &tj) {
@@ -31,8 +32,10 @@ __device__ __forceinline__ void ts_mmd_tile(int t, int T, int &m, int &ti, int &
 
 __global__ void __launch_bounds__(MTHREADS)
 ts_mmd_tiles_kernel(const float *__restrict__ X, const float *__restrict__ Y, int n, int d, int T, double *__restrict__ partial) {
-    __shared__ __align__(16) float As[MK][MT];  // component-major: a thread's four rows are one 128-bit load
-    __shared__ __align__(16) float Bs[MK][MT];
+    // component-major: a thread's four rows are one 128-bit load; rows padded by 4 floats so that the transposing stores
+    // (32 lanes = 32 components of one row) spread over 8 banks instead of hitting one
+    __shared__ __align__(16) float As[MK][MT + 4];
+    __shared__ __align__(16) float Bs[MK][MT + 4];
     __shared__ double red[MTHREADS / 32];
     int m, ti, tj;
     ts_mmd_tile((int)blockIdx.x, T, m, ti, tj);
@@ -46,7 +49,8 @@ ts_mmd_tiles_kernel(const float *__restrict__ X, const float *__restrict__ Y, in
 #pragma unroll
         for (int b = 0; b < 4; ++b) acc[a][b] = 0.f;
 
-    for (int k0 = 0; k0 < d; k0 += MK) {
+    // this CTA's share of the components: chunks of MK, dealt round-robin over the MSPLIT CTAs of the tile
+    for (int k0 = (int)blockIdx.y * MK; k0 < d; k0 += MK * MSPLIT) {
         // 64 rows x 32 components of each operand; a thread loads component (tid % 32) of rows tid / 32 + 8 p
 #pragma unroll
         for (int p = 0; p < MT / 8; ++p) {
@@ -80,21 +84,36 @@ ts_mmd_tiles_kernel(const float *__restrict__ X, const float *__restrict__ Y, in
     if (tid == 0) {
         double t = 0.0;
         for (int w = 0; w < MTHREADS / 32; ++w) t += red[w];
-        partial[blockIdx.x] = (m != 0 && tj > ti) ? 2.0 * t : t;  // the mirrored tile of a symmetric matrix
+        partial[(size_t)blockIdx.x * MSPLIT + blockIdx.y] = (m != 0 && tj > ti) ? 2.0 * t : t;  // the mirrored tile of a symmetric matrix
     }
 }
 
-__global__ void ts_mmd_final_kernel(const double *__restrict__ partial, int n, int T, double *__restrict__ out) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    const int tri = T * (T + 1) / 2;
-    double sxy = 0.0, sxx = 0.0, syy = 0.0;
-    for (int t = 0; t < T * T; ++t) sxy += partial[t];
-    for (int t = 0; t < tri; ++t) sxx += partial[T * T + t];
-    for (int t = 0; t < tri; ++t) syy += partial[T * T + tri + t];
-    out[0] = (2.0 * sxy - sxx - syy) / ((double)n * (double)n);
-    out[1] = sxy;
-    out[2] = sxx;
-    out[3] = syy;
+// Fixed-order reduction of the per-CTA partials: thread t adds partials t, t + 256, ... of a matrix in that order, then
+// the 256 thread sums are added in index order by a fixed tree -- the same bits on every run.
+__global__ void __launch_bounds__(256) ts_mmd_final_kernel(const double *__restrict__ partial, int n, int T, double *__restrict__ out) {
+    __shared__ double red[3][256];
+    const int tri = T * (T + 1) / 2, tid = threadIdx.x;
+    const int first[3] = {0, T * T * MSPLIT, (T * T + tri) * MSPLIT}, count[3] = {T * T * MSPLIT, tri * MSPLIT, tri * MSPLIT};
+#pragma unroll
+    for (int m = 0; m < 3; ++m) {
+        double s = 0.0;
+        for (int i = tid; i < count[m]; i += 256) s += partial[first[m] + i];
+        red[m][tid] = s;
+    }
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (tid < o)
+#pragma unroll
+            for (int m = 0; m < 3; ++m) red[m][tid] += red[m][tid + o];
+        __syncthreads();
+    }
+    if (tid == 0) {
+        const double sxy = red[0][0], sxx = red[1][0], syy = red[2][0];
+        out[0] = (2.0 * sxy - sxx - syy) / ((double)n * (double)n);
+        out[1] = sxy;
+        out[2] = sxx;
+        out[3] = syy;
+    }
 }
 
 // store-only fill (measurement aid: what a pure 128-bit store stream reaches on this GPU, beside the copy peak)
@@ -107,14 +126,14 @@ __global__ void __launch_bounds__(256) ts_fill_kernel(float4 *__restrict__ dst, 
 
 size_t ts_mmd_partial_count(int n) {
     const size_t T = ((size_t)n + MT - 1) / MT;
-    return T * T + T * (T + 1);
+    return (T * T + T * (T + 1)) * MSPLIT;
 }
 
 cudaError_t ts_launch_mmd(const float *d_x, const float *d_y, int n, int d, double *d_partial, double *d_out, cudaStream_t st) {
     const int T = (n + MT - 1) / MT;
     const unsigned tiles = (unsigned)(T * T + T * (T + 1));
-    ts_mmd_tiles_kernel<<<tiles, MTHREADS, 0, st>>>(d_x, d_y, n, d, T, d_partial);
-    ts_mmd_final_kernel<<<1, 32, 0, st>>>(d_partial, n, T, d_out);
+    ts_mmd_tiles_kernel<<<dim3(tiles, MSPLIT), MTHREADS, 0, st>>>(d_x, d_y, n, d, T, d_partial);
+    ts_mmd_final_kernel<<<1, 256, 0, st>>>(d_partial, n, T, d_out);
     return cudaGetLastError();
 }
 
