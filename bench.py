@@ -25,11 +25,6 @@ sys.path.insert(0, ROOT)
 METRIC = "audio samples/sec"
 UNIT = "samples/s"
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
-# Measured saturated throughput of the audible-sample instruction mix (the kernel's own loop body, no memory, 8 warps per
-# SM sub-partition; profiles/r02_audio_bounds.md): cycles per warp-unit of 640 samples per sub-partition.
-BODY_CYCLES_PER_UNIT = 1082.0
-UNIT_SAMPLES = 640
-SMSPS = 148 * 4
 
 
 def measured_peak():
@@ -174,6 +169,19 @@ def device_records(ts, W, wl, dev):
     return torch.from_numpy(h).to(dev)
 
 
+_ALU_PEAK = {}
+
+
+def alu_peak(ts):
+    """Audible samples/s the SM pipes sustain on the audio kernel's own sample loop (ts_time_alu_bound: the same device
+    function, no memory, no CTA turnover, 8 warps per sub-partition), measured once per process: MUFU.SIN variant of the
+    square/saw sine (taken by 93 % of the voices) and polynomial variant."""
+    if not _ALU_PEAK:
+        _ALU_PEAK["fastsin"] = max(ts.ts_time_alu_bound(True, 64) for _ in range(3))
+        _ALU_PEAK["poly"] = max(ts.ts_time_alu_bound(False, 64) for _ in range(3))
+    return _ALU_PEAK
+
+
 def kernel_roofline(ts, wl, rec, audio_ring, sm_hz, reps):
     """Per-kernel device times (CUDA events around `reps` back-to-back launches of each, ts_time_kernels), the active
     (non-silent) sample fraction, and the two bounds of the audio kernel."""
@@ -188,14 +196,15 @@ def kernel_roofline(ts, wl, rec, audio_ring, sm_hz, reps):
     peak, peak_src = measured_peak()
     out_bytes = B * N * 4
     achieved = out_bytes / (aud * 1e-3) / 1e9
-    alu_peak = SMSPS * UNIT_SAMPLES / BODY_CYCLES_PER_UNIT * sm_hz          # audible samples/s the SMs can compute
+    peaks = alu_peak(ts)
+    alu_pk = peaks["fastsin"]                                               # the higher of the two: a conservative fraction
     alu_ach = stats["active_samples"] / (aud * 1e-3)
     return {"audio_kernel_ms": aud, "control_kernel_ms": ctl, "achieved_gbs": achieved, "frac": achieved / peak,
             "peak": peak, "peak_source": peak_src, "active_sample_fraction": active, "chunks": stats["chunks"],
-            "alu_bound": {"bound": "alu", "what": "audible samples/s at the measured saturated throughput of the kernel's own "
-                          "instruction mix (1082 cycles per 640-sample warp-unit per SM sub-partition, 592 sub-partitions; "
-                          "profiles/r02_audio_bounds.md)", "achieved": alu_ach, "peak": alu_peak, "unit": "audible samples/s",
-                          "frac": alu_ach / alu_peak}}
+            "alu_bound": {"bound": "alu", "what": "audible samples/s the SM pipes sustain on the kernel's own sample loop "
+                          "(ts_time_alu_bound, measured in this run: same device function, no memory, no CTA turnover, 8 warps "
+                          "per sub-partition; MUFU.SIN variant; DESIGN.md 5.2)", "achieved": alu_ach, "peak": alu_pk,
+                          "peak_polynomial_sine_variant": peaks["poly"], "unit": "audible samples/s", "frac": alu_ach / alu_pk}}
 
 
 def measure_config(ts, W, torch, name, dev, sm_hz):

@@ -188,6 +188,12 @@ int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, flo
  * launches between one pair of CUDA events on the set stream -> *host_ms per launch.  What a pure store stream reaches on
  * this GPU, quoted beside the copy peak the roofline uses.  Synchronises. */
 int ts_time_fill(void *d_dst, size_t bytes, int reps, float *host_ms);
+/* Measurement aid: the ALU bound of the audible part, measured.  Runs the audio kernel's own sample loop (S9..S14: the
+ * same device function, 20 samples per thread and pass, `reps` passes) with no control table, no global stores and no CTA
+ * turnover at 8 warps per SM sub-partition, and returns the audible samples per second the SM pipes sustain with that
+ * instruction mix (fastsin: the MUFU.SIN variant of the square/saw sine taken by voices with k <= 1024, else the
+ * polynomial one).  Synchronises. */
+int ts_time_alu_bound(int fastsin, int reps, double *host_samples_per_s);
 /* Counters of the LAST ts_render (host): [0] kernels launched, [1] voice chunks,
  * [2] audio samples in the active (non-silent) prefix summed over voices (counted only while timing is
  * enabled with ts_set_timing; valid after ts_sync). */

@@ -770,6 +770,29 @@ int ts_time_fill(void *d_dst, size_t bytes, int reps, float *host_ms) {
     return TS_OK;
 }
 
+int ts_time_alu_bound(int fastsin, int reps, double *host_samples_per_s) {
+    if (!host_samples_per_s) return fail(TS_ENULL, "NULL argument%s");
+    if (reps <= 0) return fail(TS_EINVAL, "reps must be positive%s");
+    for (auto &e : S.ev)
+        if (!e) TS_CUDA(cudaEventCreate(&e));
+    cudaStream_t st = S.lane[0].stream;
+    float *sink = nullptr;
+    TS_CUDA(cudaMalloc(&sink, 1024 * sizeof(float)));
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    TS_CUDA(ts_launch_body_bench(fastsin, reps, sink, st));  // warm-up
+    TS_CUDA(cudaEventRecord(S.ev[0], st));
+    TS_CUDA(ts_launch_body_bench(fastsin, reps, sink, st));
+    TS_CUDA(cudaEventRecord(S.ev[1], st));
+    TS_CUDA(cudaEventSynchronize(S.ev[1]));
+    float ms = 0.f;
+    TS_CUDA(cudaEventElapsedTime(&ms, S.ev[0], S.ev[1]));
+    cudaFree(sink);
+    *host_samples_per_s = (double)sms * 1024.0 * (double)reps * TS_RUN / ((double)ms * 1e-3);
+    return TS_OK;
+}
+
 int ts_set_timing(int enable) {
     S.timing = enable != 0;
     return TS_OK;

@@ -315,7 +315,51 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
     }  // tiles of this CTA
 }
 
+// Measurement aid: the sample loop of the audio kernel (ts_render_run, the same device function) on its own -- no control
+// table, no global stores, no CTA turnover, 8 warps per SM sub-partition -- `reps` runs of 20 samples per thread.  What
+// the SM pipes can do with this instruction mix: the ALU bound of the audible part.
+template <int FASTSIN>
+__global__ void __launch_bounds__(1024, 1)
+ts_body_bench_kernel(float *__restrict__ sink, int reps, uint32_t nk0, uint32_t nk1, float shape, float tanh_c, uint32_t one_bits,
+                     double w0) {
+    extern __shared__ __align__(128) float4 bstage[];
+    float4 *my = &bstage[threadIdx.x * (TS_RUN / 4)];
+    uint2 *my16 = reinterpret_cast<uint2 *>(my);
+    nk0 = __reduce_or_sync(0xffffffffu, nk0);  // warp-uniform for the compiler, as blockIdx-derived values are in the real kernel
+    nk1 = __reduce_or_sync(0xffffffffu, nk1);
+    double P1 = MAGIC32 + 0.1 * threadIdx.x, P2 = MAGIC33 + 0.07 * threadIdx.x;
+    const double w1 = w0 * (1 + threadIdx.x), w2 = 1.3 * w0 * (1 + threadIdx.x);
+#pragma unroll 1
+    for (int rep = 0; rep < reps; ++rep) {
+        ts_render_run<TS_F32, FASTSIN>(P1, w1, 1e-7, P2, w2, -2e-7, 0.3f, 0.2f, 0.1f, 1e-4f, -1e-4f, 2e-4f,
+                                       (uint32_t)(rep * 5 + threadIdx.x * 77 + blockIdx.x), nk0, nk1, shape, tanh_c, one_bits, my, my16);
+        P1 += 20.0 * w1;
+        P2 += 20.0 * w2;
+    }
+    __syncthreads();
+    float s = 0.f;
+    for (int g = 0; g < TS_RUN / 4; ++g) s += my[g].x + my[g].y + my[g].z + my[g].w;
+    if (s == 123.456f) sink[threadIdx.x] = s;  // keeps the loop alive; never true in practice
+}
+
 }  // namespace
+
+cudaError_t ts_launch_body_bench(int fastsin, int reps, float *d_sink, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(ts_body_bench_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 1024 * TS_RUN * 4);
+        cudaFuncSetAttribute(ts_body_bench_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 1024 * TS_RUN * 4);
+        attr = true;
+    }
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (fastsin)
+        ts_body_bench_kernel<1><<<sms, 1024, 1024 * TS_RUN * 4, st>>>(d_sink, reps, 123u, 456u, 0.4f, 20.f, 0x3f800000u, 1e-3);
+    else
+        ts_body_bench_kernel<0><<<sms, 1024, 1024 * TS_RUN * 4, st>>>(d_sink, reps, 123u, 456u, 0.4f, 20.f, 0x3f800000u, 1e-3);
+    return cudaGetLastError();
+}
 
 cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, void *audio, int fmt,
                             int mode, int tails, double *dbg_phase, cudaStream_t st) {
