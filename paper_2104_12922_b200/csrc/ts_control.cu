@@ -161,42 +161,84 @@ __device__ __forceinline__ void ts_block_scan2(unsigned long long &a, unsigned l
     __syncthreads();  // scratch may be reused
 }
 
+constexpr int TS_CTL_THREADS = 128;
+constexpr int TS_CTL_IC = TS_CTL_THREADS - 1;  // control intervals per chunk (the last thread is the halo tick)
+
 // ---- decoupled look-back over the chunk aggregates of one voice ------------------------------------
+// A slot is two 16-byte words, each a Q0.64 sum with the launch epoch beside it: one 128-bit store publishes a word,
+// one 128-bit load reads value and flag together (aligned 16-byte accesses are single transactions), so neither side
+// needs a fence -- the same packing CUB's single-word tile descriptors use.
+struct __align__(16) ts_agg_word {
+    unsigned long long s;
+    unsigned int flag;  // == launch epoch once s is valid
+    unsigned int pad;
+};
 struct __align__(16) ts_agg {
-    unsigned long long s[2];
-    unsigned int flag;  // == launch epoch once s[] is valid
-    unsigned int pad[3];
+    ts_agg_word w[2];
 };
 static_assert(sizeof(ts_agg) == 32, "ts_agg layout");
 
 __device__ __forceinline__ void ts_publish(ts_agg *slot, unsigned long long a, unsigned long long b, unsigned int epoch) {
-    slot->s[0] = a;
-    slot->s[1] = b;
-    __threadfence();
-    *reinterpret_cast<volatile unsigned int *>(&slot->flag) = epoch;
+    uint4 w0, w1;
+    w0.x = (unsigned int)a; w0.y = (unsigned int)(a >> 32); w0.z = epoch; w0.w = 0u;
+    w1.x = (unsigned int)b; w1.y = (unsigned int)(b >> 32); w1.z = epoch; w1.w = 0u;
+    asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(&slot->w[0]), "r"(w0.x), "r"(w0.y), "r"(w0.z), "r"(w0.w) : "memory");
+    asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(&slot->w[1]), "r"(w1.x), "r"(w1.y), "r"(w1.z), "r"(w1.w) : "memory");
 }
-// Threads 0..c-1 each fetch one predecessor's aggregate; the sums are combined through shared memory.
-// A predecessor always has a lower block index, so it has been dispatched before this CTA (in-order dispatch of a 1-D
-// grid); the wait is nevertheless bounded: after TS_SPIN_LIMIT polls (about a second) the CTA raises the launch's error
+// A predecessor always has a lower linear block index, so it has been dispatched before this CTA (in-order dispatch);
+// the wait is nevertheless bounded: after TS_SPIN_LIMIT polls (about a second) the thread raises the launch's error
 // flag and goes on with what it has, and the host turns the flag into TS_ECUDA at the next ts_sync().
 constexpr int TS_SPIN_LIMIT = 1 << 24;
-__device__ __forceinline__ void ts_lookback(const ts_agg *slots, int c, unsigned int epoch, unsigned long long *acc /*smem[2]*/,
-                                            unsigned int *err) {
-    for (int i = threadIdx.x; i < c; i += blockDim.x) {
-        const ts_agg *p = slots + i;
-        int spins = 0;
-        while (*reinterpret_cast<const volatile unsigned int *>(&p->flag) != epoch) {
-            __nanosleep(40);
-            if (++spins > TS_SPIN_LIMIT) {
-                atomicExch(err, 1u);
-                break;
-            }
+__device__ __forceinline__ void ts_wait_slot(const ts_agg *p, unsigned int epoch, unsigned int *err, unsigned long long &a,
+                                             unsigned long long &b) {
+    uint4 v0, v1;
+    int spins = 0;
+    for (;;) {  // both words in flight at once: one L2 round trip when the predecessor has already published
+        asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v0.x), "=r"(v0.y), "=r"(v0.z), "=r"(v0.w) : "l"(&p->w[0]) : "memory");
+        asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v1.x), "=r"(v1.y), "=r"(v1.z), "=r"(v1.w) : "l"(&p->w[1]) : "memory");
+        if (v0.z == epoch && v1.z == epoch) break;
+        __nanosleep(40);
+        if (++spins > TS_SPIN_LIMIT) {
+            atomicExch(err, 1u);
+            break;
         }
-        __threadfence();
-        const unsigned long long a = *reinterpret_cast<const volatile unsigned long long *>(&p->s[0]);
-        const unsigned long long b = *reinterpret_cast<const volatile unsigned long long *>(&p->s[1]);
-        atomicAdd(&acc[0], a);
-        atomicAdd(&acc[1], b);
+    }
+    a = ((unsigned long long)v0.y << 32) | v0.x;
+    b = ((unsigned long long)v1.y << 32) | v1.x;
+}
+// Sum of the aggregates of chunks 0 .. c-1 (mod 2^64): every thread fetches its share of the predecessors, the partial
+// sums meet through warp shuffles and one shared-memory word per warp.  Call with all threads; the totals are in
+// sm[0 .. nw) and sm[32 .. 32 + nw) after the caller's next __syncthreads().
+__device__ __forceinline__ void ts_lookback(const ts_agg *slots, int c, unsigned int epoch, unsigned long long *sm /*[64]*/,
+                                            unsigned int *err) {
+    unsigned long long a = 0ull, b = 0ull;
+    if ((int)(threadIdx.x & ~31u) < c) {  // warps without a predecessor to fetch skip the reduction
+        for (int i = threadIdx.x; i < c; i += blockDim.x) {
+            unsigned long long x, y;
+            ts_wait_slot(&slots[i], epoch, err, x, y);
+            a += x;
+            b += y;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a += __shfl_down_sync(0xffffffffu, a, o);
+            b += __shfl_down_sync(0xffffffffu, b, o);
+        }
+    }
+    if ((threadIdx.x & 31) == 0) {
+        sm[threadIdx.x >> 5] = a;
+        sm[32 + (threadIdx.x >> 5)] = b;
+    }
+}
+__device__ __forceinline__ void ts_lookback_total(const unsigned long long *sm, int c, unsigned long long &a, unsigned long long &b) {
+    a = sm[0];
+    b = sm[32];
+    if (c > 32) {  // more than one warp fetched predecessors
+#pragma unroll
+        for (int w = 1; w < TS_CTL_THREADS / 32; ++w) {
+            a += sm[w];
+            b += sm[32 + w];
+        }
     }
 }
 
@@ -223,8 +265,6 @@ __device__ __forceinline__ double ts_lfo_mix(double p, const double *wn) {
     return v;
 }
 
-constexpr int TS_CTL_THREADS = 128;
-constexpr int TS_CTL_IC = TS_CTL_THREADS - 1;  // control intervals per chunk (the last thread is the halo tick)
 
 // ---- per-voice setup: one CTA per voice ----------------------------------------------------------------------------
 // S1 (optional: the fused sampler of the streaming path), S2/S3 parameter map, the constants every tick needs, the
@@ -366,7 +406,7 @@ ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, 
     __shared__ ts_voice_consts V;
     __shared__ ts_math_tables MT;
     __shared__ unsigned long long scan_sm[64];
-    __shared__ unsigned long long acc[4];
+    __shared__ unsigned long long lb_sm[64];
     __shared__ double2 pitch[TS_CTL_THREADS];
     __shared__ double Es[6][TS_CTL_THREADS];
 
@@ -397,7 +437,6 @@ ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, 
         reinterpret_cast<double *>(&MT)[tid] = reinterpret_cast<const double *>(&c_math)[tid];
     if (tid < (int)(sizeof(ts_voice_consts) / 16))
         reinterpret_cast<uint4 *>(&V)[tid] = __ldg(reinterpret_cast<const uint4 *>(vc + v) + tid);
-    if (tid < 4) acc[tid] = 0ull;
     __syncthreads();
     const double *h = V.h;
     const long long J = (N + R - 1) / R;  // control intervals that hold samples (PHASES = 1: R == TS_R)
@@ -427,9 +466,11 @@ ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, 
     }
     ts_block_scan2(dq1, dq2, scan_sm);  // exclusive prefix inside the chunk
     if (tid == TS_CTL_IC) ts_publish(&agg_q[c], dq1, dq2, epoch);  // halo thread: sum over the chunk's own 127 ticks
-    ts_lookback(agg_q, c, epoch, &acc[0], err);
+    ts_lookback(agg_q, c, epoch, lb_sm, err);
     __syncthreads();
-    const unsigned long long q1 = ts_frac_q64(h[34]) + acc[0] + dq1, q2 = ts_frac_q64(h[42]) + acc[1] + dq2;
+    unsigned long long lbq1, lbq2;
+    ts_lookback_total(lb_sm, c, lbq1, lbq2);
+    const unsigned long long q1 = ts_frac_q64(h[34]) + lbq1 + dq1, q2 = ts_frac_q64(h[42]) + lbq2 + dq2;
     // the halo tick is written by the next chunk unless that chunk has nothing to do
     const bool own = (tid < TS_CTL_IC) || (j0 + TS_CTL_IC >= jsil) || (c == NC - 1);
     double M[5] = {0, 0, 0, 0, 0};
@@ -488,10 +529,12 @@ ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, 
     }
     ts_block_scan2(s1, s2, scan_sm);
     if (tid == TS_CTL_IC) ts_publish(&agg_p[c], s1, s2, epoch);
-    ts_lookback(agg_p, c, epoch, &acc[2], err);
+    ts_lookback(agg_p, c, epoch, lb_sm, err);
     __syncthreads();
     if (act) {
-        const unsigned long long P1 = ts_frac_q64(h[70]) + acc[2] + s1, P2 = ts_frac_q64(h[73]) + acc[3] + s2;
+        unsigned long long lbp1, lbp2;
+        ts_lookback_total(lb_sm, c, lbp1, lbp2);
+        const unsigned long long P1 = ts_frac_q64(h[70]) + lbp1 + s1, P2 = ts_frac_q64(h[73]) + lbp2 + s2;
         double2 *d2 = reinterpret_cast<double2 *>(&tab[j]);
         d2[0] = make_double2(ts_q64_to_double(P1), inc[0]);
         d2[1] = make_double2(e1[0], g20[0]);
