@@ -204,7 +204,8 @@ def kernel_roofline(ts, wl, rec, audio_ring, sm_hz, reps):
             "alu_bound": {"bound": "alu", "what": "audible samples/s the SM pipes sustain on the kernel's own sample loop "
                           "(ts_time_alu_bound, measured in this run: same device function, no memory, no CTA turnover, 8 warps "
                           "per sub-partition; MUFU.SIN variant; DESIGN.md 5.2)", "achieved": alu_ach, "peak": alu_pk,
-                          "peak_polynomial_sine_variant": peaks["poly"], "unit": "audible samples/s", "frac": alu_ach / alu_pk}}
+                          "peak_polynomial_sine_variant": peaks["poly"], "unit": "audible samples/s", "frac": alu_ach / alu_pk,
+                          "cycles_per_warp_instruction_per_subpartition": ts.ts_time_pipes()}}
 
 
 def measure_config(ts, W, torch, name, dev, sm_hz):

@@ -194,6 +194,11 @@ int ts_time_fill(void *d_dst, size_t bytes, int reps, float *host_ms);
  * instruction mix (fastsin: the MUFU.SIN variant of the square/saw sine taken by voices with k <= 1024, else the
  * polynomial one).  Synchronises. */
 int ts_time_alu_bound(int fastsin, int reps, double *host_samples_per_s);
+/* Measurement aid: issue rate of the instruction kinds the audio kernel is made of, each alone, 8 warps per SM
+ * sub-partition with 8 independent chains per thread.  host_rates[k] = cycles per warp instruction per sub-partition:
+ * [0] FFMA, [1] FFMA2 (packed fp32x2), [2] IMAD.WIDE.U32 (the Philox multiply), [3] LOP3, [4] DFMA, [5] MUFU.SIN with its
+ * range-reduction FMUL, [6] MUFU.EX2, [7] I2FP.  DESIGN.md 5.2 derives the kernel's pipe budget from them.  Synchronises. */
+int ts_time_pipes(double host_rates[8]);
 /* Counters of the LAST ts_render (host): [0] kernels launched, [1] voice chunks,
  * [2] audio samples in the active (non-silent) prefix summed over voices (counted only while timing is
  * enabled with ts_set_timing; valid after ts_sync). */

@@ -31,7 +31,7 @@ class _Out(C.Structure):
 EXPORTS = ["ts_sample_params", "ts_render", "ts_render_fmt", "ts_render_host", "ts_render_host_fmt", "ts_corpus_render",
            "ts_corpus_render_fmt", "ts_corpus_open", "ts_corpus_next", "ts_corpus_close", "ts_corpus_is_test", "ts_num_samples",
            "ts_num_ticks", "ts_num_ticks_r", "ts_set_stream", "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes",
-           "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_time_kernels", "ts_time_fill", "ts_time_alu_bound", "ts_last_kernel_ms",
+           "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_time_kernels", "ts_time_fill", "ts_time_alu_bound", "ts_time_pipes", "ts_last_kernel_ms",
            "ts_last_stats", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_debug_noise_u32", "ts_debug_controls",
            "ts_debug_phase"]
 TS_F32, TS_F16, TS_BF16 = 0, 1, 2
@@ -74,6 +74,7 @@ def lib():
     L.ts_num_ticks_r.restype = C.c_int64
     L.ts_time_fill.argtypes = [vp, C.c_size_t, i32, vp]
     L.ts_time_alu_bound.argtypes = [i32, i32, vp]
+    L.ts_time_pipes.argtypes = [vp]
     L.ts_render_controls_r.argtypes = [vp, i32, i32, f64, i32, vp]
     L.ts_mmd_l1.argtypes = [vp, vp, i32, i32, vp]
     L.ts_corpus_is_test.argtypes = [u64]
@@ -362,6 +363,17 @@ def ts_time_alu_bound(fastsin: bool, reps: int = 64) -> float:
     _use_current_stream(_torch().device("cuda", _torch().cuda.current_device()))
     _check(lib().ts_time_alu_bound(int(fastsin), reps, C.byref(v)))
     return float(v.value)
+
+
+PIPE_NAMES = ["FFMA", "FFMA2", "IMAD.WIDE.U32", "LOP3", "DFMA", "MUFU.SIN+FMUL", "MUFU.EX2", "I2FP"]
+
+
+def ts_time_pipes() -> dict:
+    """-> {instruction kind: cycles per warp instruction per SM sub-partition}, each kind issued alone."""
+    r = (C.c_double * 8)()
+    _use_current_stream(_torch().device("cuda", _torch().cuda.current_device()))
+    _check(lib().ts_time_pipes(r))
+    return {n: float(r[i]) for i, n in enumerate(PIPE_NAMES)}
 
 
 def ts_render_controls_r(params, sr: int, seconds: float, R: int):

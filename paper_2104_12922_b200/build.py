@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtsynth.so")
-SOURCES = ["ts_api.cu", "ts_sample.cu", "ts_control.cu", "ts_audio.cu", "ts_mmd.cu"]
+SOURCES = ["ts_api.cu", "ts_sample.cu", "ts_control.cu", "ts_audio.cu", "ts_mmd.cu", "ts_measure.cu"]
 HEADERS = [os.path.join(CSRC, "ts_common.cuh"), os.path.join(CSRC, "ts_math.cuh"), os.path.join(HERE, "..", "include", "tsynth.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]

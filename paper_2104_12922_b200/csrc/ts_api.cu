@@ -793,6 +793,12 @@ int ts_time_alu_bound(int fastsin, int reps, double *host_samples_per_s) {
     return TS_OK;
 }
 
+int ts_time_pipes(double host_rates[8]) {
+    if (!host_rates) return fail(TS_ENULL, "NULL argument%s");
+    TS_CUDA(ts_measure_pipes(host_rates, S.lane[0].stream));
+    return TS_OK;
+}
+
 int ts_set_timing(int enable) {
     S.timing = enable != 0;
     return TS_OK;

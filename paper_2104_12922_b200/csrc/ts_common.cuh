@@ -81,6 +81,8 @@ cudaError_t ts_upload_math_tables(cudaStream_t st);
 size_t ts_control_agg_bytes(int B, int K);  // look-back slots; must be zero before the first launch
 cudaError_t ts_launch_body_bench(int fastsin, int reps, float *d_sink, cudaStream_t st);  // the audio kernel's sample loop alone
 cudaError_t ts_launch_fill(void *d_dst, size_t bytes, cudaStream_t st);  // store-only fill kernel (measurement aid)
+constexpr int TS_NPIPES = 8;
+cudaError_t ts_measure_pipes(double host_rates[TS_NPIPES], cudaStream_t st);  // issue rates of the audio kernel's instruction kinds
 cudaError_t ts_launch_mmd(const float *d_x, const float *d_y, int n, int d, double *d_partial, double *d_out, cudaStream_t st);
 size_t ts_mmd_partial_count(int n);
 // epoch: a value never used before on this `agg` buffer (flags from older launches then read as "not ready")

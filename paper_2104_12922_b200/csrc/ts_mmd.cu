@@ -116,12 +116,6 @@ __global__ void __launch_bounds__(256) ts_mmd_final_kernel(const double *__restr
     }
 }
 
-// store-only fill (measurement aid: what a pure 128-bit store stream reaches on this GPU, beside the copy peak)
-__global__ void __launch_bounds__(256) ts_fill_kernel(float4 *__restrict__ dst, size_t n16) {
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride) dst[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-}
-
 }  // namespace
 
 size_t ts_mmd_partial_count(int n) {
@@ -134,10 +128,5 @@ cudaError_t ts_launch_mmd(const float *d_x, const float *d_y, int n, int d, doub
     const unsigned tiles = (unsigned)(T * T + T * (T + 1));
     ts_mmd_tiles_kernel<<<dim3(tiles, MSPLIT), MTHREADS, 0, st>>>(d_x, d_y, n, d, T, d_partial);
     ts_mmd_final_kernel<<<1, 256, 0, st>>>(d_partial, n, T, d_out);
-    return cudaGetLastError();
-}
-
-cudaError_t ts_launch_fill(void *d_dst, size_t bytes, cudaStream_t st) {
-    ts_fill_kernel<<<148 * 32, 256, 0, st>>>(static_cast<float4 *>(d_dst), bytes / 16);
     return cudaGetLastError();
 }
