@@ -37,7 +37,7 @@ struct ts_corpus_state {  // the streaming iterator (ts_corpus_open / next / clo
     bool open = false;
     ts_corpus_cfg cfg;
     int64_t N = 0;
-    uint64_t next_out = 0, next_render = 0;  // batch indices
+    uint64_t first = 0, next_out = 0, next_render = 0;  // batch indices
     cudaEvent_t ready[TS_MAX_RING] = {};     // slot rendered
     cudaEvent_t consumed = nullptr;          // the caller's stream has passed the previous hand-out
 };
@@ -51,8 +51,11 @@ struct ts_state {
     ts_lane lane[TS_LANES];
     ts_lane *cur = &lane[0];
     cudaEvent_t fork = nullptr;
-    cudaStream_t hi = nullptr, lo = nullptr;  // the streaming calls' internal streams
-    uint64_t stream_count = 0;                // batches issued on the internal streams (picks lane 1 / 2)
+    // the streaming calls' internal streams: one high-priority (setup, control) and one low-priority (audio) stream per
+    // streaming lane, so that consecutive chunks overlap completely (kernel launch gaps included)
+    cudaStream_t hi[2] = {nullptr, nullptr}, lo[2] = {nullptr, nullptr};
+    cudaEvent_t batch_done[TS_MAX_RING][2] = {};  // audio of batch (count % TS_MAX_RING) issued on lo[x] has finished
+    cudaEvent_t join_ev[4] = {nullptr, nullptr, nullptr, nullptr};
     // host staging for ts_render_host
     void *stage = nullptr;
     size_t stage_bytes = 0;
@@ -344,42 +347,62 @@ int ensure_streams() {
     if (S.fork) return TS_OK;
     int lo_p = 0, hi_p = 0;
     TS_CUDA(cudaDeviceGetStreamPriorityRange(&lo_p, &hi_p));  // numerically lower = higher priority
-    TS_CUDA(cudaStreamCreateWithPriority(&S.hi, cudaStreamNonBlocking, hi_p));
-    TS_CUDA(cudaStreamCreateWithPriority(&S.lo, cudaStreamNonBlocking, lo_p));
-    for (int l = 1; l < TS_LANES; ++l) {
-        S.lane[l].stream = S.hi;
-        S.lane[l].audio_stream = S.lo;
-        TS_CUDA(cudaEventCreateWithFlags(&S.lane[l].ctl_done, cudaEventDisableTiming));
-        TS_CUDA(cudaEventCreateWithFlags(&S.lane[l].aud_done, cudaEventDisableTiming));
+    for (int x = 0; x < 2; ++x) {
+        TS_CUDA(cudaStreamCreateWithPriority(&S.hi[x], cudaStreamNonBlocking, hi_p));
+        TS_CUDA(cudaStreamCreateWithPriority(&S.lo[x], cudaStreamNonBlocking, lo_p));
+        S.lane[1 + x].stream = S.hi[x];
+        S.lane[1 + x].audio_stream = S.lo[x];
+        TS_CUDA(cudaEventCreateWithFlags(&S.lane[1 + x].ctl_done, cudaEventDisableTiming));
+        TS_CUDA(cudaEventCreateWithFlags(&S.lane[1 + x].aud_done, cudaEventDisableTiming));
     }
+    for (auto &e : S.join_ev) TS_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    for (auto &b : S.batch_done)
+        for (auto &e : b) TS_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     TS_CUDA(cudaEventCreateWithFlags(&S.fork, cudaEventDisableTiming));
     return TS_OK;
 }
 
-// Both internal streams start after everything already queued on the caller's stream.
+// All internal streams start after everything already queued on the caller's stream.
 int fork_streams() {
     TS_CUDA(cudaEventRecord(S.fork, S.lane[0].stream));
-    TS_CUDA(cudaStreamWaitEvent(S.hi, S.fork, 0));
-    TS_CUDA(cudaStreamWaitEvent(S.lo, S.fork, 0));
+    for (int x = 0; x < 2; ++x) {
+        TS_CUDA(cudaStreamWaitEvent(S.hi[x], S.fork, 0));
+        TS_CUDA(cudaStreamWaitEvent(S.lo[x], S.fork, 0));
+    }
     return TS_OK;
 }
 
 // A batch on the internal streams (forked by the caller): the voice chunks of the batch alternate between the two
 // streaming lanes, setup + control on `hi`, audio on `lo`, so that the control stage of one chunk overlaps the audio
 // stage of the previous one -- across the chunks of a batch as well as across batches.
-int stream_batch(ts_voice *p, sample_spec smp, int B, int sr, double seconds, int fmt, void *a, float *params_human) {
+// seq: position of the batch in its sequence (chunk j of the batch runs on lane (seq + j) & 1).  n_ring > 0: the batch
+// goes into the ring slot that batch seq - n_ring wrote: that batch's audio, possibly on the other audio stream, must
+// have finished first.
+int stream_batch(ts_voice *p, sample_spec smp, int B, int sr, double seconds, int fmt, void *a, float *params_human, uint64_t seq = 0,
+                 int n_ring = 0) {
     int64_t N;
     int K;
     int rc = check_sizes(B, sr, seconds, &N, &K);
     if (rc) return rc;
     const int Bc = chunk_voices(B, K);
+    // Single-chunk batches alternate strictly between the two lanes; with an even ring a slot is then always written
+    // on the same audio stream and stream order covers the hazard.
+    const bool same_stream = (Bc >= B) && (n_ring % 2 == 0);
+    if (n_ring > 0 && !same_stream) {
+        const uint64_t k = (uint64_t)(n_ring < TS_MAX_RING ? n_ring : TS_MAX_RING);
+        if (seq >= k) {
+            cudaEvent_t *ev = S.batch_done[(seq - k) % TS_MAX_RING];
+            for (int x = 0; x < 2; ++x)
+                for (int y = 0; y < 2; ++y) TS_CUDA(cudaStreamWaitEvent(S.lo[x], ev[y], 0));
+        }
+    }
     const size_t es = fmt_bytes(fmt);
     const bool timing = S.timing;
     S.timing = false;  // per-kernel events would serialise the streams
     int64_t launches = 0, chunks = 0;
     for (int b0 = 0; b0 < B && rc == TS_OK; b0 += Bc) {
         const int nb = (B - b0 < Bc) ? (B - b0) : Bc;
-        S.cur = &S.lane[1 + (int)(S.stream_count++ & 1)];
+        S.cur = &S.lane[1 + (int)((seq + (uint64_t)chunks) & 1)];
         rc = render_impl(p + b0, sample_spec{smp.on, smp.seed, smp.g0 + (uint64_t)b0}, nb, sr, seconds, fmt,
                          static_cast<char *>(a) + (size_t)b0 * (size_t)N * es,
                          params_human ? params_human + (size_t)b0 * TS_NPARAM : nullptr, 0, nullptr);
@@ -390,15 +413,19 @@ int stream_batch(ts_voice *p, sample_spec smp, int B, int sr, double seconds, in
     S.cur = &S.lane[0];
     S.stats[0] = launches;
     S.stats[1] = chunks;
+    if (rc == TS_OK && n_ring > 0 && !same_stream)
+        for (int x = 0; x < 2; ++x) TS_CUDA(cudaEventRecord(S.batch_done[seq % TS_MAX_RING][x], S.lo[x]));
     return rc;
 }
 
-// The caller's stream continues after both internal streams.
+// The caller's stream continues after all internal streams.
 int join_streams() {
-    TS_CUDA(cudaEventRecord(S.lane[1].ctl_done, S.hi));
-    TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.lane[1].ctl_done, 0));
-    TS_CUDA(cudaEventRecord(S.lane[2].ctl_done, S.lo));
-    TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.lane[2].ctl_done, 0));
+    for (int x = 0; x < 2; ++x) {
+        TS_CUDA(cudaEventRecord(S.join_ev[2 * x], S.hi[x]));
+        TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.join_ev[2 * x], 0));
+        TS_CUDA(cudaEventRecord(S.join_ev[2 * x + 1], S.lo[x]));
+        TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.join_ev[2 * x + 1], 0));
+    }
     return TS_OK;
 }
 
@@ -408,9 +435,13 @@ int corpus_issue(uint64_t batch) {  // render `batch` into its slot and record t
     const size_t es = fmt_bytes(C.cfg.fmt);
     const int rc = stream_batch(C.cfg.d_params_ring + (size_t)slot * (size_t)C.cfg.B,
                                 sample_spec{true, C.cfg.seed, batch * (uint64_t)C.cfg.B}, C.cfg.B, C.cfg.sr, C.cfg.seconds, C.cfg.fmt,
-                                static_cast<char *>(C.cfg.d_audio_ring) + (size_t)slot * (size_t)C.cfg.B * (size_t)C.N * es, nullptr);
+                                static_cast<char *>(C.cfg.d_audio_ring) + (size_t)slot * (size_t)C.cfg.B * (size_t)C.N * es, nullptr,
+                                batch - C.first, C.cfg.n_ring);
     if (rc) return rc;
-    TS_CUDA(cudaEventRecord(C.ready[slot], S.lo));
+    // the slot is ready when the batch's audio on BOTH audio streams has finished
+    TS_CUDA(cudaEventRecord(S.join_ev[1], S.lo[1]));
+    TS_CUDA(cudaStreamWaitEvent(S.lo[0], S.join_ev[1], 0));
+    TS_CUDA(cudaEventRecord(C.ready[slot], S.lo[0]));
     return TS_OK;
 }
 
@@ -524,7 +555,7 @@ int ts_corpus_render_fmt(uint64_t seed, uint64_t first_batch, int n_batches, int
     for (int i = 0; i < n_batches && rc == TS_OK; ++i) {
         const size_t slot = (size_t)(i % n_ring);
         rc = stream_batch(d_params_ring + slot * (size_t)B, sample_spec{true, seed, (first_batch + (uint64_t)i) * (uint64_t)B}, B, sr,
-                          seconds, fmt, static_cast<char *>(d_audio_ring) + slot * (size_t)B * (size_t)N * es, nullptr);
+                          seconds, fmt, static_cast<char *>(d_audio_ring) + slot * (size_t)B * (size_t)N * es, nullptr, (uint64_t)i, n_ring);
         launches += S.stats[0];
     }
     const int rj = join_streams();
@@ -555,7 +586,7 @@ int ts_corpus_open(const ts_corpus_cfg *host_cfg, uint64_t first_batch) {
     ts_corpus_state &C = S.corpus;
     C.cfg = *host_cfg;
     C.N = N;
-    C.next_out = C.next_render = first_batch;
+    C.first = C.next_out = C.next_render = first_batch;
     for (int i = 0; i < host_cfg->n_ring; ++i)
         if (!C.ready[i]) TS_CUDA(cudaEventCreateWithFlags(&C.ready[i], cudaEventDisableTiming));
     if (!C.consumed) TS_CUDA(cudaEventCreateWithFlags(&C.consumed, cudaEventDisableTiming));
@@ -577,8 +608,10 @@ int ts_corpus_next(ts_corpus_batch *host_out) {
     // slot not in flight: the batch n_ring - 1 ahead of the one handed out now goes into it, ordered after the caller's
     // stream (both internal streams wait for it).
     TS_CUDA(cudaEventRecord(C.consumed, S.lane[0].stream));
-    TS_CUDA(cudaStreamWaitEvent(S.lo, C.consumed, 0));
-    TS_CUDA(cudaStreamWaitEvent(S.hi, C.consumed, 0));
+    for (int x = 0; x < 2; ++x) {
+        TS_CUDA(cudaStreamWaitEvent(S.lo[x], C.consumed, 0));
+        TS_CUDA(cudaStreamWaitEvent(S.hi[x], C.consumed, 0));
+    }
     const int rc = corpus_issue(C.next_render++);
     if (rc) return rc;
     const uint64_t b = C.next_out++;
@@ -598,8 +631,10 @@ int ts_corpus_close(void) {
     ts_corpus_state &C = S.corpus;
     if (!C.open) return TS_OK;
     C.open = false;
-    TS_CUDA(cudaStreamSynchronize(S.hi));
-    TS_CUDA(cudaStreamSynchronize(S.lo));
+    for (int x = 0; x < 2; ++x) {
+        TS_CUDA(cudaStreamSynchronize(S.hi[x]));
+        TS_CUDA(cudaStreamSynchronize(S.lo[x]));
+    }
     return TS_OK;
 }
 
@@ -681,8 +716,15 @@ void ts_shutdown(void) {
         L.stream = keep;
     }
     if (S.fork) { cudaEventDestroy(S.fork); S.fork = nullptr; }
-    if (S.hi) { cudaStreamDestroy(S.hi); S.hi = nullptr; }
-    if (S.lo) { cudaStreamDestroy(S.lo); S.lo = nullptr; }
+    for (int x = 0; x < 2; ++x) {
+        if (S.hi[x]) { cudaStreamDestroy(S.hi[x]); S.hi[x] = nullptr; }
+        if (S.lo[x]) { cudaStreamDestroy(S.lo[x]); S.lo[x] = nullptr; }
+    }
+    for (auto &e : S.join_ev)
+        if (e) { cudaEventDestroy(e); e = nullptr; }
+    for (auto &b : S.batch_done)
+        for (auto &e : b)
+            if (e) { cudaEventDestroy(e); e = nullptr; }
     if (S.stage) cudaFree(S.stage);
     if (S.mmd_ws) cudaFree(S.mmd_ws);
     for (auto &e : S.ev)
