@@ -143,11 +143,19 @@ bool nebula_supported(int sr) {
 // Does the active nebula leave a long exactly-silent tail in a buffer of `seconds`?  Every voice is silent after
 // duration + the longest release of the four audible envelopes (H6); if even the longest such voice leaves a fifth of
 // the buffer silent, the audio kernel lets its audible CTAs write the tails (ts_audio.cu, TAIL = 1).
-int tails_expected(double seconds) {
+double nebula_t_end() {  // no voice of the active nebula is audible after this time (u is clamped to [0,1], S3)
     const ts_range *n = S.nebula;
     auto hi = [&](int i) { return fmax(n[i].lo, n[i].hi); };
-    const double t_end = hi(1) + fmax(fmax(hi(5), hi(10)), fmax(hi(15), hi(25)));
-    return t_end < 0.8 * seconds;
+    return hi(1) + fmax(fmax(hi(5), hi(10)), fmax(hi(15), hi(25)));
+}
+int tails_expected(double seconds) { return nebula_t_end() < 0.8 * seconds; }
+// Upper bound of n_act over all voices (samples): the setup kernel's first silent tick is the first j with
+// j R / sr - D >= rl_max, so j <= ceil(t_end sr / R) (+1 tick against the rounding of the division); the audio kernel
+// launches no CTAs for tiles that cannot be audible.
+int64_t max_audible_samples(int sr, int64_t N) {
+    const double ticks = ceil(nebula_t_end() * (double)sr / (double)TS_R) + 1.0;
+    const double n = ticks * (double)TS_R;
+    return (n < (double)N) ? (int64_t)n : N;
 }
 
 int chunk_voices(int B, int K) {
@@ -306,7 +314,8 @@ int render_impl(ts_voice *d_params, sample_spec smp, int B, int sr, double secon
                                 params_human ? params_human + (size_t)b0 * TS_NPARAM : nullptr,
                                 want_stats ? ln.d_active : nullptr, (mode == 1 || mode == 2 || mode == 3) ? 1 : 0, ln.stream));
         TS_CUDA(ts_launch_control(vc, nb, sr, R, N, K, table, agg, ln.epoch,
-                                  (mode == 3 || mode == 4) ? dbg + (size_t)b0 * 5 * K : nullptr, with_table ? 1 : 0, ln.d_err,
+                                  (mode == 3 || mode == 4) ? dbg + (size_t)b0 * 5 * K : nullptr, with_table ? 1 : 0,
+                                  (mode == 0) ? max_audible_samples(sr, N) : (int64_t)-1, ln.d_err,
                                   ln.stream));
         launches += 2;
         if (timed) TS_CUDA(cudaEventRecord(S.ev[1], ln.stream));
@@ -318,7 +327,8 @@ int render_impl(ts_voice *d_params, sample_spec smp, int B, int sr, double secon
         }
         if (mode <= 2) {
             TS_CUDA(ts_launch_audio(table, hdr, nb, N, K, audio ? static_cast<char *>(audio) + (size_t)b0 * N * es : nullptr, fmt,
-                                    mode, tails_expected(seconds), (mode == 1 || mode == 2) ? dbg + (size_t)b0 * N : nullptr, ast));
+                                    mode, tails_expected(seconds), max_audible_samples(sr, N),
+                                    (mode == 1 || mode == 2) ? dbg + (size_t)b0 * N : nullptr, ast));
             ++launches;
         }
         if (ast != ln.stream) {  // the next control launch on this workspace will wait for this audio kernel
@@ -775,13 +785,13 @@ int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, flo
                 ln.epoch = 1;
             }
             TS_CUDA(ts_launch_setup(const_cast<ts_voice *>(d_params) + b0, 0, 0, 0, nb, sr, TS_R, N, K, vc, hdr, nullptr, nullptr, 0, st));
-            TS_CUDA(ts_launch_control(vc, nb, sr, TS_R, N, K, table, agg, ln.epoch, nullptr, 1, ln.d_err, st));
+            TS_CUDA(ts_launch_control(vc, nb, sr, TS_R, N, K, table, agg, ln.epoch, nullptr, 1, max_audible_samples(sr, N), ln.d_err, st));
         }
         TS_CUDA(cudaEventRecord(S.ev[1], st));
         for (int r = 0; r < reps; ++r)
             TS_CUDA(ts_launch_audio(table, hdr, nb, N, K,
                                     d_audio_ring + (size_t)(r % n_ring) * (size_t)B * (size_t)N + (size_t)b0 * (size_t)N, TS_F32,
-                                    0, tails, nullptr, st));
+                                    0, tails, max_audible_samples(sr, N), nullptr, st));
         TS_CUDA(cudaEventRecord(S.ev[2], st));
         TS_CUDA(cudaEventSynchronize(S.ev[2]));
         float x = 0.f, y = 0.f;

@@ -362,11 +362,14 @@ cudaError_t ts_launch_body_bench(int fastsin, int reps, float *d_sink, cudaStrea
 }
 
 cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, void *audio, int fmt,
-                            int mode, int tails, double *dbg_phase, cudaStream_t st) {
+                            int mode, int tails, int64_t n_audible_max, double *dbg_phase, cudaStream_t st) {
     const int64_t tiles = (N + TS_TILE - 1) / TS_TILE;
     // two tiles per CTA once the launch is large enough to fill the GPU many times over
     const int tpc = (mode == 0 && tiles * B >= 12000) ? 2 : 1;
-    const int64_t ty = (tiles + tpc - 1) / tpc;
+    // with TAIL = 1 the silent tiles have no CTA of their own: launch only the tiles that can be audible
+    const int64_t tiles_aud = (mode == 0 && tails) ? (n_audible_max + TS_TILE - 1) / TS_TILE : tiles;
+    const int64_t tl = (tiles_aud < tiles) ? (tiles_aud > 0 ? tiles_aud : 1) : tiles;
+    const int64_t ty = (tl + tpc - 1) / tpc;
     if (ty > 0x7fffffffLL || (ty > 65535 && B > 65535)) return cudaErrorInvalidValue;
     const int swap = ty > 65535;
     const dim3 g = swap ? dim3((unsigned)ty, (unsigned)B) : dim3((unsigned)B, (unsigned)ty);

@@ -93,11 +93,12 @@ cudaError_t ts_launch_setup(ts_voice *d_params, int sample, uint64_t seed, uint6
                             ts_voice_consts *vc, ts_vhdr *hdr, float *params_human, unsigned long long *d_active, int full,
                             cudaStream_t st);
 // phases != 0: also the S9 tick-level phase scan and the control table (needed by the audio kernel); phases == 0 stops
-// after the modulation mixer (control-rate rendering on its own).  d_err: device flag raised if a look-back wait gives up
+// after the modulation mixer (control-rate rendering on its own).  n_audible_max >= 0: no voice is audible at or after this sample (chunks past it are not launched); d_err: device flag raised if a look-back wait gives up
 cudaError_t ts_launch_control(const ts_voice_consts *vc, int B, int sr, int R, int64_t N, int K, ts_tick *table, void *agg,
-                              unsigned int epoch, double *dbg_ctl, int phases, unsigned int *d_err, cudaStream_t st);
+                              unsigned int epoch, double *dbg_ctl, int phases, int64_t n_audible_max, unsigned int *d_err, cudaStream_t st);
 // mode 0: audio; mode 1 / 2: write the phase of VCO 1 / 2 (fp64 cycles) to dbg_phase instead.
-// tails != 0: long silent tails are expected (nebula + buffer length), let the audible CTAs write them asynchronously
+// tails != 0: long silent tails are expected (nebula + buffer length), let the audible CTAs write them asynchronously;
+// n_audible_max: no voice is audible at or after this sample (then no CTA is launched for those tiles)
 // fmt: TS_F32 / TS_F16 / TS_BF16 output samples
 cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, void *audio, int fmt,
-                            int mode, int tails, double *dbg_phase, cudaStream_t st);
+                            int mode, int tails, int64_t n_audible_max, double *dbg_phase, cudaStream_t st);

@@ -557,13 +557,21 @@ cudaError_t ts_launch_setup(ts_voice *d_params, int sample, uint64_t seed, uint6
 }
 
 cudaError_t ts_launch_control(const ts_voice_consts *vc, int B, int sr, int R, int64_t N, int K, ts_tick *table, void *agg,
-                              unsigned int epoch, double *dbg_ctl, int phases, unsigned int *d_err, cudaStream_t st) {
+                              unsigned int epoch, double *dbg_ctl, int phases, int64_t n_audible_max, unsigned int *d_err, cudaStream_t st) {
     const int J = K - 1;
     int NC = (J + TS_CTL_IC - 1) / TS_CTL_IC;
     if (NC < 1) NC = 1;
-    if (NC > 65535 && B > 65535) return cudaErrorInvalidValue;
-    const int swap = NC > 65535;
-    const dim3 grid = swap ? dim3((unsigned)NC, (unsigned)B) : dim3((unsigned)B, (unsigned)NC);
+    // chunks that start at or after the last tick any voice can be audible at are dead for every voice: not launched
+    // (unless the caller wants the zeros of the control-rate output written, or every tick evaluated)
+    int NCL = NC;
+    if (!dbg_ctl && n_audible_max >= 0) {
+        const int64_t jmax = (n_audible_max + R - 1) / R + 1;
+        const int64_t need = (jmax + TS_CTL_IC - 1) / TS_CTL_IC;
+        if (need < NCL) NCL = (int)(need > 0 ? need : 1);
+    }
+    if (NCL > 65535 && B > 65535) return cudaErrorInvalidValue;
+    const int swap = NCL > 65535;
+    const dim3 grid = swap ? dim3((unsigned)NCL, (unsigned)B) : dim3((unsigned)B, (unsigned)NCL);
     if (phases && R != TS_R) return cudaErrorInvalidValue;  // the audio kernel's geometry is built on R = 100
     if (phases)
         ts_control_kernel<1><<<grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
