@@ -69,7 +69,9 @@ int ts_sample_params(uint64_t seed, uint64_t batch_index, int B, ts_voice *d_par
  * linear upsampling -> phase-accumulating sine and square/saw VCOs + Philox white noise -> VCAs ->
  * mixer -> out.audio.  u outside [0,1] (or NaN) is clamped to [0,1].  d_params is read only.
  * Errors: TS_ENULL (d_params or out.audio NULL), TS_EINVAL (sizes; or the active nebula allows an
- * oscillator increment beyond the supported 2^18/TS_R cycles per sample at this sr). */
+ * oscillator increment beyond the supported 2^18/TS_R cycles per sample at this sr: the check is on the nebula's
+ * maximum pitch, midi.hi + tune.hi + |depth|, not on the voices of the call, so the default nebula -- 291 cycles per
+ * sample at 44.1 kHz -- is refused below sr = 4.9 kHz). */
 int ts_render(const ts_voice *d_params, int B, int sr, double seconds, ts_out out);
 
 /* Output sample formats.  The path computes in fp32 (fp64 / Q0.64 for the phase chain) whatever the format; TS_F16 and
@@ -166,7 +168,7 @@ int64_t ts_num_ticks(int64_t N);
 
 int ts_set_stream(void *cuda_stream);              /* cudaStream_t; NULL = legacy default stream   */
 int ts_default_nebula(ts_range host_out78[TS_NPARAM]); /* host copy of the built-in table S2        */
-int ts_set_nebula(const ts_range *host_in78);      /* host table; NULL restores the default        */
+int ts_set_nebula(const ts_range *host_in78);      /* host table; NULL restores the default.  TS_EINVAL: non-finite entries, curve <= 0, or a negative range for a weight (LFO shapes 35..39, 43..47; modulation mixer 48..67) */
 size_t ts_workspace_bytes(int B, int sr, double seconds); /* device bytes ts_render will hold      */
 const char *ts_last_error(void);                   /* host string, owned by the library            */
 int ts_sync(void);                                 /* cudaStreamSynchronize on the set stream; TS_ECUDA if a kernel raised the device error flag */

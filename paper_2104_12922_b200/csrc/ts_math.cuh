@@ -3,6 +3,10 @@
 // correctly-rounded-over-the-whole-range versions: ~35 instructions per pow instead of ~250, and no
 // fp64 divisions.  Tables (768 B) are generated on the host in long double when the library starts
 // and staged in shared memory by the kernel.
+// Technique: the table-driven log2 (mantissa window [0.6875, 1.375) split into 2^-5 steps, table of reciprocals and
+// logarithms of the interval centres, short polynomial in r = z/c - 1) and the exp2 with a `1.5 * 2^52` shift to split
+// exponent, table index and remainder are the scheme used by open libm implementations (ARM optimized-routines /
+// musl `log2`, `exp2`); table sizes, polynomial degrees and coefficients here are this code's own.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
