@@ -159,7 +159,7 @@ __device__ __forceinline__ void ts_render_run(double P1, double w1, const double
 // which costs ~14 % of an SM's time at one tile per CTA; small launches keep TPC = 1 so that the last wave stays short).
 template <int MODE, int TAIL, int FMT, int TPC>
 __global__ void __launch_bounds__(TS_AUDIO_THREADS)
-ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ hdr, int B, long long N, int K,
+ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ hdr, int B, int N, int K,
                 void *__restrict__ audio_, double *__restrict__ dbg_phase, int aligned, uint32_t one_bits, int swap) {
     __shared__ __align__(128) float4 stage[TS_TILE / 4];
     __shared__ __align__(128) float4 zero[(MODE == 0 && TAIL) ? TS_TILE / 4 : 4];  // source of the tail's zero-fill bulk copies
@@ -169,20 +169,21 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
     // 2-D grid, no integer division: x = voice, y = tile (x runs fastest: time-major dispatch, the audible tiles of all
     // voices go first); swapped when a voice has more than 65535 tiles
     const int voice = swap ? blockIdx.y : blockIdx.x;
-    const long long tile_first = (swap ? blockIdx.x : blockIdx.y) * (long long)TPC;
+    // N < 2^31 (ts_api.cu check_sizes): sample, run and tile indices are 32-bit, only byte offsets are 64-bit
+    const int tile_first = (int)(swap ? blockIdx.x : blockIdx.y) * TPC;
     const int tid = threadIdx.x;
     const ts_vhdr hd = hdr[voice];
-    const long long T = (N + TS_TILE - 1) / TS_TILE;
+    const int T = (N + TS_TILE - 1) / TS_TILE;
     bool zeroed = false;  // the zero buffer is filled once per CTA
 #pragma unroll 1
     for (int tt = 0; tt < TPC; ++tt) {
-    const long long tile = tile_first + tt;
+    const int tile = tile_first + tt;
     if (tile >= T) return;
     if (TPC > 1 && tt > 0) __syncthreads();  // the previous tile's bulk copy has read the staging tile (thread 0 waited)
-    const long long n_tile0 = tile * TS_TILE;
-    const long long rem = N - n_tile0;
-    const int count = (rem < TS_TILE) ? (int)rem : TS_TILE;  // samples of this tile inside the buffer
-    char *row = audio + ((size_t)voice * N + n_tile0) * ES;
+    const int n_tile0 = tile * TS_TILE;
+    const int rem = N - n_tile0;
+    const int count = (rem < TS_TILE) ? rem : TS_TILE;  // samples of this tile inside the buffer
+    char *row = audio + ((size_t)voice * (size_t)N + (size_t)n_tile0) * ES;
 
     if (MODE == 0 && !TAIL && n_tile0 >= hd.n_act) {  // silent tile: exact zeros (S4 release over; pin P9)
         if (aligned) {
@@ -200,10 +201,10 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
         // CTAs of their own: audible tile t of a voice with A audible tiles writes the silent tiles A + t, A + t + A, ...
         // as asynchronous bulk copies of a zero buffer (TMA engine), issued BEFORE its arithmetic, so that the stores
         // of the tails overlap the issue-bound arithmetic of the audible part instead of following it.
-        long long A = ((long long)hd.n_act + TS_TILE - 1) / TS_TILE;
+        int A = (hd.n_act + TS_TILE - 1) / TS_TILE;
         if (A < 1) A = 1;  // a voice with no audible sample: tile 0 renders zeros and owns the whole tail
         if (tile >= A) return;  // and so are all later tiles of this voice
-        char *vrow = audio + (size_t)voice * N * ES;
+        char *vrow = audio + (size_t)voice * (size_t)N * ES;
         if (A + tile >= T) {
             // no silent tile falls to this CTA
         } else if (aligned) {
@@ -216,33 +217,33 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
             }
             if ((tid & 31) == 0) {  // lane 0 of each warp issues every fourth copy
                 const uint32_t zs = (uint32_t)__cvta_generic_to_shared(zero);
-                for (long long tz = A + tile + (tid >> 5) * A; tz < T; tz += (TS_AUDIO_THREADS / 32) * A) {
-                    const long long rz = N - tz * TS_TILE;
-                    ts_bulk_issue(vrow + tz * TS_TILE * ES, zs, ((rz < TS_TILE) ? (uint32_t)rz : (uint32_t)TS_TILE) * ES);
+                for (int tz = A + tile + (tid >> 5) * A; tz < T; tz += (TS_AUDIO_THREADS / 32) * A) {
+                    const int rz = N - tz * TS_TILE;
+                    ts_bulk_issue(vrow + (size_t)tz * (TS_TILE * ES), zs, ((rz < TS_TILE) ? (uint32_t)rz : (uint32_t)TS_TILE) * ES);
                 }
                 asm volatile("cp.async.bulk.commit_group;" ::: "memory");
             }
         } else {
-            for (long long tz = A + tile; tz < T; tz += A) {
-                const long long rz = N - tz * TS_TILE;
-                const int cz = (rz < TS_TILE) ? (int)rz : TS_TILE;
+            for (int tz = A + tile; tz < T; tz += A) {
+                const int rz = N - tz * TS_TILE;
+                const int cz = (rz < TS_TILE) ? rz : TS_TILE;
                 if (FMT == TS_F32)
-                    for (int i = tid; i < cz; i += TS_AUDIO_THREADS) reinterpret_cast<float *>(vrow)[tz * TS_TILE + i] = 0.f;
+                    for (int i = tid; i < cz; i += TS_AUDIO_THREADS) reinterpret_cast<float *>(vrow)[(size_t)tz * TS_TILE + i] = 0.f;
                 else
-                    for (int i = tid; i < cz; i += TS_AUDIO_THREADS) reinterpret_cast<unsigned short *>(vrow)[tz * TS_TILE + i] = 0;
+                    for (int i = tid; i < cz; i += TS_AUDIO_THREADS) reinterpret_cast<unsigned short *>(vrow)[(size_t)tz * TS_TILE + i] = 0;
             }
         }
     }
 
-    const long long r = tile * TS_AUDIO_THREADS + tid;  // run index inside the voice
-    const long long n0 = r * TS_RUN;
+    const int r = tile * TS_AUDIO_THREADS + tid;  // run index inside the voice
+    const int n0 = r * TS_RUN;
     // this thread's 20 samples inside the staging tile: 80 bytes (fp32) or 40 bytes (16-bit formats), conflict-free
     float4 *my = &stage[tid * (TS_RUN / 4)];
     uint2 *my16 = reinterpret_cast<uint2 *>(reinterpret_cast<char *>(stage) + tid * (TS_RUN * 2));
 
     if (n0 < hd.n_act || (MODE != 0 && n0 < N)) {
-        const int j = (int)(r / TS_RUNS_PER_TICK);
-        const int q = (int)(r - (long long)j * TS_RUNS_PER_TICK);
+        const int j = r / TS_RUNS_PER_TICK;
+        const int q = r - j * TS_RUNS_PER_TICK;
         const ts_tick *tk = table + (size_t)voice * K + j;
         const double2 *t2 = reinterpret_cast<const double2 *>(tk);
         const double2 v0 = __ldg(t2 + 0), v1 = __ldg(t2 + 1), v2 = __ldg(t2 + 2), v3 = __ldg(t2 + 3);
@@ -281,9 +282,9 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
                                       one_bits, my, my16);
         } else {
             for (int i = 0; i < TS_RUN; ++i) {
-                const long long n = n0 + i;
+                const int n = n0 + i;
                 const double ph = (MODE == 1) ? (P1 - MAGIC32) : (P2 - MAGIC33);
-                if (n < N) dbg_phase[(size_t)voice * N + n] = ph - floor(ph);
+                if (n < N) dbg_phase[(size_t)voice * (size_t)N + n] = ph - floor(ph);
                 P1 += w1; w1 = fma(w1, e1a, w1);
                 P2 += w2; w2 = fma(w2, e1b, w2);
             }
@@ -377,7 +378,7 @@ cudaError_t ts_launch_audio(const ts_tick *table, const ts_vhdr *hdr, int B, int
     const int per16 = (fmt == TS_F32) ? 4 : 8;
     const int aligned = (N % per16 == 0) && ((reinterpret_cast<uintptr_t>(audio) & 15u) == 0);
 #define TS_LAUNCH(MODE, TAIL, FMT, TPC) \
-    ts_audio_kernel<MODE, TAIL, FMT, TPC><<<g, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, N, K, audio, dbg_phase, aligned, 0x3f800000u, swap)
+    ts_audio_kernel<MODE, TAIL, FMT, TPC><<<g, TS_AUDIO_THREADS, 0, st>>>(table, hdr, B, (int)N, K, audio, dbg_phase, aligned, 0x3f800000u, swap)
 #define TS_LAUNCH_T(TAIL, FMT) do { if (tpc == 2) TS_LAUNCH(0, TAIL, FMT, 2); else TS_LAUNCH(0, TAIL, FMT, 1); } while (0)
     if (mode == 0) {
         if (fmt == TS_F32) { if (tails) TS_LAUNCH_T(1, TS_F32); else TS_LAUNCH_T(0, TS_F32); }
