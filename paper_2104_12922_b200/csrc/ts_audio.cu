@@ -173,6 +173,10 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
     const int tile_first = (int)(swap ? blockIdx.x : blockIdx.y) * TPC;
     const int tid = threadIdx.x;
     const ts_vhdr hd = hdr[voice];
+    // TAIL = 1: a CTA whose first tile is past the voice's last audible sample has nothing to do (its tiles are written
+    // by the voice's audible CTAs); it leaves before any other arithmetic.  Tile 0 always stays (it owns the tail of a
+    // voice with no audible sample).
+    if (MODE == 0 && TAIL && tile_first > 0 && tile_first * TS_TILE >= hd.n_act) return;
     const int T = (N + TS_TILE - 1) / TS_TILE;
     bool zeroed = false;  // the zero buffer is filled once per CTA
 #pragma unroll 1
