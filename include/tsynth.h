@@ -149,6 +149,13 @@ int ts_render_controls(const ts_voice *d_params, int B, int sr, double seconds, 
 int ts_render_controls_r(const ts_voice *d_params, int B, int sr, double seconds, int R, double *d_ctl);
 int64_t ts_num_ticks_r(int64_t N, int R);
 
+/* ts_render with the tick spacing chosen per call, fp32 output: R = TS_R is ts_render; R = 1 is the audio-rate-control
+ * mode of SURVEY 8(f) item 3 (every sample is a control tick: ADSRs, LFOs and the mixer are evaluated at every sample,
+ * upsampling is the identity, pin P7; reading D27).  R = 1 is a mode for studying the two-rate design (D1), not the hot
+ * path: its control table has one entry per sample (80 B), so a call is split into chunks of a few voices.  Other values
+ * of R: TS_EINVAL. */
+int ts_render_r(const ts_voice *d_params, int B, int sr, double seconds, int R, float *d_audio);
+
 /* Maximum mean discrepancy of two sets of n embeddings of dimension d with the l1 distance as the core distance
  * (Eq. 2 at P:L230; "1/nn" there is read as 1/n^2, reading D25; the paper's setting is n = 1000, d = 512,
  * P:L257):  MMD(X, Y) = (1/n^2) sum_{i,j} [ 2 |x_i - y_j|_1 - |x_i - x_j|_1 - |y_i - y_j|_1 ].

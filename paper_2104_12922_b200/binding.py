@@ -32,7 +32,7 @@ EXPORTS = ["ts_sample_params", "ts_render", "ts_render_fmt", "ts_render_host", "
            "ts_corpus_render_fmt", "ts_corpus_open", "ts_corpus_next", "ts_corpus_close", "ts_corpus_is_test", "ts_num_samples",
            "ts_num_ticks", "ts_num_ticks_r", "ts_set_stream", "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes",
            "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_time_kernels", "ts_time_fill", "ts_time_alu_bound", "ts_time_pipes", "ts_last_kernel_ms",
-           "ts_last_stats", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_debug_noise_u32", "ts_debug_controls",
+           "ts_last_stats", "ts_render_r", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_debug_noise_u32", "ts_debug_controls",
            "ts_debug_phase"]
 TS_F32, TS_F16, TS_BF16 = 0, 1, 2
 
@@ -76,6 +76,7 @@ def lib():
     L.ts_time_alu_bound.argtypes = [i32, i32, vp]
     L.ts_time_pipes.argtypes = [vp]
     L.ts_render_controls_r.argtypes = [vp, i32, i32, f64, i32, vp]
+    L.ts_render_r.argtypes = [vp, i32, i32, f64, i32, vp]
     L.ts_mmd_l1.argtypes = [vp, vp, i32, i32, vp]
     L.ts_corpus_is_test.argtypes = [u64]
     L.ts_num_samples.argtypes = [i32, f64]
@@ -374,6 +375,18 @@ def ts_time_pipes() -> dict:
     _use_current_stream(_torch().device("cuda", _torch().cuda.current_device()))
     _check(lib().ts_time_pipes(r))
     return {n: float(r[i]) for i, n in enumerate(PIPE_NAMES)}
+
+
+def ts_render_r(params, sr: int, seconds: float, R: int):
+    """ts_render with the tick spacing chosen per call (R = 100, or R = 1: audio-rate control) -> fp32 audio [B, N]."""
+    torch = _torch()
+    p = _dev_params(params)
+    B = p.shape[0]
+    N = ts_num_samples(sr, seconds)
+    out = torch.empty((B, N), dtype=torch.float32, device=p.device)
+    _use_current_stream(p.device)
+    _check(lib().ts_render_r(C.c_void_p(p.data_ptr()), B, sr, float(seconds), R, C.c_void_p(out.data_ptr())))
+    return out
 
 
 def ts_render_controls_r(params, sr: int, seconds: float, R: int):

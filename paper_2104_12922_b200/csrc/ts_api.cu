@@ -259,7 +259,7 @@ struct sample_spec {  // the fused sampler of the streaming path: draw the recor
 };
 
 // mode 0: audio (+ optional params_human); 1/2: debug phase of VCO 1/2; 3: debug controls of the audio path;
-// mode 4: control-rate rendering on its own (no oscillator stage; tick spacing R)
+// mode 4: control-rate rendering on its own (no oscillator stage; tick spacing R); mode 5: audio with R = 1
 int render_impl(ts_voice *d_params, sample_spec smp, int B, int sr, double seconds, int fmt, void *audio, float *params_human,
                 int mode, double *dbg, int R = TS_R) {
     int64_t N;
@@ -325,7 +325,10 @@ int render_impl(ts_voice *d_params, sample_spec smp, int B, int sr, double secon
             TS_CUDA(cudaEventRecord(ln.ctl_done, ln.stream));
             TS_CUDA(cudaStreamWaitEvent(ast, ln.ctl_done, 0));
         }
-        if (mode <= 2) {
+        if (mode == 5) {
+            TS_CUDA(ts_launch_audio_r1(table, hdr, nb, N, K, static_cast<float *>(audio) + (size_t)b0 * N, ast));
+            ++launches;
+        } else if (mode <= 2) {
             TS_CUDA(ts_launch_audio(table, hdr, nb, N, K, audio ? static_cast<char *>(audio) + (size_t)b0 * N * es : nullptr, fmt,
                                     mode, tails_expected(seconds), max_audible_samples(sr, N),
                                     (mode == 1 || mode == 2) ? dbg + (size_t)b0 * N : nullptr, ast));
@@ -872,6 +875,14 @@ int ts_render_controls_r(const ts_voice *d_params, int B, int sr, double seconds
     if (!d_params || !d_ctl) return fail(TS_ENULL, "NULL argument%s");
     if (R <= 0) return fail(TS_EINVAL, "R must be positive%s");
     return render_impl(const_cast<ts_voice *>(d_params), sample_spec{false, 0, 0}, B, sr, seconds, TS_F32, nullptr, nullptr, 4, d_ctl, R);
+}
+int ts_render_r(const ts_voice *d_params, int B, int sr, double seconds, int R, float *d_audio) {
+    if (!d_params || !d_audio) return fail(TS_ENULL, "NULL argument%s");
+    if (R == TS_R) return ts_render_fmt(d_params, B, sr, seconds, TS_F32, d_audio, nullptr);
+    if (R != 1) return fail(TS_EINVAL, "the audio path is built for R = 100 and R = 1%s");
+    if (S.corpus.open) return fail(TS_EINVAL, "close the corpus iterator first%s");
+    S.cur = &S.lane[0];
+    return render_impl(const_cast<ts_voice *>(d_params), sample_spec{false, 0, 0}, B, sr, seconds, TS_F32, d_audio, nullptr, 5, nullptr, 1);
 }
 int ts_render_controls(const ts_voice *d_params, int B, int sr, double seconds, double *d_ctl) {
     return ts_render_controls_r(d_params, B, sr, seconds, TS_R, d_ctl);

@@ -320,6 +320,52 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
     }  // tiles of this CTA
 }
 
+// ---- audio-rate-control mode (R = 1): every sample is a control tick, so there is no upsampling
+// (pin P7) and no recurrence: a sample's phases and gains are its own table entry.  One thread renders the four samples of
+// one Philox block.  A mode for studying the two-rate design (D1), not the hot path: plain fp32 arithmetic, the
+// relative-accuracy polynomial for the square/saw sine, 128-bit stores when the row is aligned.
+__global__ void __launch_bounds__(128)
+ts_audio_r1_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ hdr, int B, int N, int K,
+                   float *__restrict__ audio, int aligned, uint32_t one_bits) {
+    const int voice = blockIdx.y;
+    const int n0 = (blockIdx.x * 128 + threadIdx.x) * 4;
+    if (n0 >= N) return;
+    const ts_vhdr hd = hdr[voice];
+    float o[4] = {0.f, 0.f, 0.f, 0.f};
+    if (n0 < hd.n_act) {
+        uint32_t nz[4];
+        ts_philox4x32_10((uint32_t)(n0 >> 2), 0u, 0u, 1u, hd.nk0, hd.nk1, nz);  // S12
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int n = n0 + i;
+            if (n >= hd.n_act || n >= N) continue;
+            const ts_tick *tk = table + (size_t)voice * K + n;
+            const double P1 = __ldg(&tk->phi1) + MAGIC32, P2 = __ldg(&tk->phi2) + MAGIC33;
+            const float4 g = __ldg(reinterpret_cast<const float4 *>(&tk->a1));
+            const int xa = __double2loint(P1), la = __double2loint(P2), ha = __double2hiint(P2);
+            const float y1 = __sinf((float)xa * 1.4629180792671596e-9f);                                    // S10
+            const uint32_t sg = (((uint32_t)la + ((uint32_t)ha << 31)) & 0x80000000u) | one_bits;       // S11 (H4)
+            const float th = (float)la * 7.314590396335798e-10f, t2 = th * th;
+            float q = fmaf(t2, SIN_C9, SIN_C7);
+            q = fmaf(q, t2, SIN_C5);
+            q = fmaf(q, t2, SIN_C3);
+            const float sn = fmaf(th * t2, q, th);
+            const float tnh = fmaf(ts_rcp(ts_ex2(sn * hd.tanh_c) + 1.0f), -2.0f, 1.0f);
+            const float y2 = tnh * fmaf(hd.shape, __cosf(th), __uint_as_float(sg));
+            const float z = fmaf(__uint2float_rz(nz[i]), 4.656612873077393e-10f, -1.0f);                  // S12, D24
+            o[i] = fmaf(g.z, z, fmaf(g.y, y2, g.x * y1));                                                  // S13, S14
+        }
+    }
+    float *row = audio + (size_t)voice * (size_t)N;
+    if (aligned) {
+        *reinterpret_cast<float4 *>(row + n0) = make_float4(o[0], o[1], o[2], o[3]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            if (n0 + i < N) row[n0 + i] = o[i];
+    }
+}
+
 // Measurement aid: the sample loop of the audio kernel (ts_render_run, the same device function) on its own -- no control
 // table, no global stores, no CTA turnover, 8 warps per SM sub-partition -- `reps` runs of 20 samples per thread.  What
 // the SM pipes can do with this instruction mix: the ALU bound of the audible part.
@@ -363,6 +409,14 @@ cudaError_t ts_launch_body_bench(int fastsin, int reps, float *d_sink, cudaStrea
         ts_body_bench_kernel<1><<<sms, 1024, 1024 * TS_RUN * 4, st>>>(d_sink, reps, 123u, 456u, 0.4f, 20.f, 0x3f800000u, 1e-3);
     else
         ts_body_bench_kernel<0><<<sms, 1024, 1024 * TS_RUN * 4, st>>>(d_sink, reps, 123u, 456u, 0.4f, 20.f, 0x3f800000u, 1e-3);
+    return cudaGetLastError();
+}
+
+cudaError_t ts_launch_audio_r1(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, float *audio, cudaStream_t st) {
+    const int64_t gx = (N + 511) / 512;
+    if (gx > 0x7fffffffLL || B > 65535) return cudaErrorInvalidValue;
+    const int aligned = (N % 4 == 0) && ((reinterpret_cast<uintptr_t>(audio) & 15u) == 0);
+    ts_audio_r1_kernel<<<dim3((unsigned)gx, (unsigned)B), 128, 0, st>>>(table, hdr, B, (int)N, K, audio, aligned, 0x3f800000u);
     return cudaGetLastError();
 }
 

@@ -79,6 +79,8 @@ cudaError_t ts_launch_noise_debug(uint32_t k0, uint32_t k1, uint64_t n0, int cou
 cudaError_t ts_upload_nebula(const ts_range *host78, cudaStream_t st);
 cudaError_t ts_upload_math_tables(cudaStream_t st);
 size_t ts_control_agg_bytes(int B, int K);  // look-back slots; must be zero before the first launch
+// the audio-rate-control mode: table entries are per SAMPLE (control kernel with R = 1)
+cudaError_t ts_launch_audio_r1(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, float *audio, cudaStream_t st);
 cudaError_t ts_launch_body_bench(int fastsin, int reps, float *d_sink, cudaStream_t st);  // the audio kernel's sample loop alone
 cudaError_t ts_launch_fill(void *d_dst, size_t bytes, cudaStream_t st);  // store-only fill kernel (measurement aid)
 constexpr int TS_NPIPES = 8;

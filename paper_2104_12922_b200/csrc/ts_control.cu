@@ -396,7 +396,9 @@ ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64
     }
 }
 
-// PHASES = 1: controls + the S9 tick-level phase scan + the control table of the audio kernel;
+// PHASES = 1: controls + the S9 tick-level phase scan + the control table of the audio kernel (R = TS_R);
+// PHASES = 2: the same for the audio-rate-control mode R = 1 (an interval is one sample: its phase advance is the
+//             increment itself, no geometric sums);
 // PHASES = 0: stops after the modulation mixer (control-rate rendering on its own: no interval sums, no second scan)
 template <int PHASES>
 __global__ void __launch_bounds__(TS_CTL_THREADS)
@@ -511,6 +513,12 @@ ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, 
         for (int o = 0; o < 2; ++o) {
             const double pa = o ? p0.y : p0.x, pb = o ? p1.y : p1.x;
             const double inc0_ = f0 * ts_exp2((pa - 69.0) * (1.0 / 12.0), &MT);
+            if (PHASES == 2) {  // R = 1: the interval holds one sample
+                const unsigned long long sf1 = ts_frac_q64(inc0_);
+                if (o) { s2 = sf1; inc[1] = inc0_; e1[1] = 0.0; g20[1] = 1.0; }
+                else   { s1 = sf1; inc[0] = inc0_; e1[0] = 0.0; g20[0] = 1.0; }
+                continue;
+            }
             const double x1 = ts_expm1_small((pb - pa) * (0.69314718055994530942 / (12.0 * TS_R)));  // rho - 1
             // geometric sums by doubling: x_m = rho^m - 1, g_m = 1 + rho + ... + rho^(m-1)
             const double x2 = x1 * (2.0 + x1), x4 = x2 * (2.0 + x2);
@@ -572,8 +580,11 @@ cudaError_t ts_launch_control(const ts_voice_consts *vc, int B, int sr, int R, i
     if (NCL > 65535 && B > 65535) return cudaErrorInvalidValue;
     const int swap = NCL > 65535;
     const dim3 grid = swap ? dim3((unsigned)NCL, (unsigned)B) : dim3((unsigned)B, (unsigned)NCL);
-    if (phases && R != TS_R) return cudaErrorInvalidValue;  // the audio kernel's geometry is built on R = 100
-    if (phases)
+    if (phases && R != TS_R && R != 1) return cudaErrorInvalidValue;  // the audio kernels are built on R = 100 and R = 1
+    if (phases && R == 1)
+        ts_control_kernel<2><<<grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
+                                                             static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err, swap);
+    else if (phases)
         ts_control_kernel<1><<<grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
                                                                        static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err, swap);
     else

@@ -614,3 +614,31 @@ def test_lookback_stress_bitwise_repeatable(T):
         assert torch.equal(T.ts_render(dev, wl.sr, wl.seconds), first), it
     T.ts_sync()
     T.ts_set_nebula(None)
+
+
+def test_audio_rate_control_mode_r1(T):
+    """SURVEY 8(f) item 3, the R = 1 mode of the AUDIO path (reading D27): every sample is a control tick.  Against the
+    oracle's render_voice_r(R = 1) on C2's first voices at C2's length (176 401 ticks per voice), plus a ragged case; and
+    it must differ from the R = 100 render (the two-rate design is a definition, D1), while R = 100 through the same call
+    is ts_render bit for bit."""
+    import torch
+    wl, neb, u, nk, dev = setup_workload(T, "C2")
+    B = 6
+    d6 = dev[:B].contiguous()
+    g = T.ts_render_r(d6, wl.sr, wl.seconds, 1).cpu().numpy()
+    o = np.stack([O.render_voice_r(u[b], nk[b], wl.sr, wl.N, 1, neb)["audio"] for b in range(B)])
+    print("R=1 worst:", assert_parity(g, o, "R=1"))
+    for b in range(B):
+        nzo = np.flatnonzero(o[b])
+        last = nzo[-1] + 1 if nzo.size else 0
+        assert not np.any(g[b, last:]), b
+    g100 = T.ts_render(d6, wl.sr, wl.seconds)
+    assert torch.equal(T.ts_render_r(d6, wl.sr, wl.seconds, 100), g100)
+    assert np.abs(g - g100.cpu().numpy()).max() > 1e-3
+    sr, seconds = 48000, 0.0501                                              # N = 2405: not a multiple of 4
+    N = O.num_samples(sr, seconds)
+    g = T.ts_render_r(d6[:2].contiguous(), sr, seconds, 1).cpu().numpy()
+    o = np.stack([O.render_voice_r(u[b], nk[b], sr, N, 1, neb)["audio"] for b in range(2)])
+    assert_parity(g, o, "R=1 ragged")
+    with pytest.raises(T.TsynthError):
+        T.ts_render_r(d6, wl.sr, wl.seconds, 7)
