@@ -1,6 +1,6 @@
 // ts_control.cu -- control-rate stage (S2..S7) and the tick-level phase scan of S9.
 //
-// Flat grid over (voice, chunk of 127 control intervals); 128 threads, one control tick each (the last
+// 2-D grid over (voice, chunk of 255 control intervals); 256 threads, one control tick each (the last
 // thread's tick is the halo shared with the next chunk).  Per tick (tau_j = j*R/sr, S5) a thread evaluates
 // the six ADSRs in closed form (S4), the two LFOs (S6; each with its rate and amp ADSR,
 // P:L123) and the modulation mixer (S7), all in fp64 because the two pitch rows feed the oscillator phase
@@ -155,13 +155,17 @@ __device__ __forceinline__ void ts_block_scan2(unsigned long long &a, unsigned l
     if (lane == 31) { sm[wid] = ia; sm[32 + wid] = ib; }
     __syncthreads();
     unsigned long long oa = 0, ob = 0;
-    for (int w = 0; w < wid && w < nw; ++w) { oa += sm[w]; ob += sm[32 + w]; }  // <= 3 terms for 128 threads
+    for (int w = 0; w < wid && w < nw; ++w) { oa += sm[w]; ob += sm[32 + w]; }  // <= 7 terms for 256 threads
     a = oa + ia - a;
     b = ob + ib - b;
     __syncthreads();  // scratch may be reused
 }
 
-constexpr int TS_CTL_THREADS = 128;
+#ifndef TS_CTL_THREADS_N
+#define TS_CTL_THREADS_N 256
+#endif
+constexpr int TS_CTL_THREADS = TS_CTL_THREADS_N;  // 255 control intervals per chunk: 128 / 256 / 512 measured 32.9 / 32.4 / 32.5 us per C2 step, 64 worse
+constexpr int TS_SETUP_THREADS = 128;  // the setup kernel's thread roles are laid out for 128 threads
 constexpr int TS_CTL_IC = TS_CTL_THREADS - 1;  // control intervals per chunk (the last thread is the halo tick)
 
 // ---- decoupled look-back over the chunk aggregates of one voice ------------------------------------
@@ -270,7 +274,7 @@ __device__ __forceinline__ double ts_lfo_mix(double p, const double *wn) {
 // S1 (optional: the fused sampler of the streaming path), S2/S3 parameter map, the constants every tick needs, the
 // first tick at which the voice is silent for good, and the voice header of the audio kernel.  Everything here used to
 // be recomputed by every chunk CTA of the control kernel (2.3 us each); now it runs once per voice.
-__global__ void __launch_bounds__(TS_CTL_THREADS)
+__global__ void __launch_bounds__(TS_SETUP_THREADS)
 ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64_t g0, int B, int sr, int R, long long N, int K,
                 ts_voice_consts *__restrict__ vc, ts_vhdr *__restrict__ hdr, float *__restrict__ params_human,
                 unsigned long long *__restrict__ d_active, int full) {
@@ -435,10 +439,10 @@ ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, 
     ts_agg *agg_q = agg + ((size_t)v * NC) * 2, *agg_p = agg_q + NC;
 
     // ---- stage the math tables and the voice's constants ----
-    if (tid < (int)(sizeof(ts_math_tables) / 8))
-        reinterpret_cast<double *>(&MT)[tid] = reinterpret_cast<const double *>(&c_math)[tid];
-    if (tid < (int)(sizeof(ts_voice_consts) / 16))
-        reinterpret_cast<uint4 *>(&V)[tid] = __ldg(reinterpret_cast<const uint4 *>(vc + v) + tid);
+    for (int i = tid; i < (int)(sizeof(ts_math_tables) / 8); i += TS_CTL_THREADS)
+        reinterpret_cast<double *>(&MT)[i] = reinterpret_cast<const double *>(&c_math)[i];
+    for (int i = tid; i < (int)(sizeof(ts_voice_consts) / 16); i += TS_CTL_THREADS)
+        reinterpret_cast<uint4 *>(&V)[i] = __ldg(reinterpret_cast<const uint4 *>(vc + v) + i);
     __syncthreads();
     const double *h = V.h;
     const long long J = (N + R - 1) / R;  // control intervals that hold samples (PHASES = 1: R == TS_R)
@@ -467,7 +471,7 @@ ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, 
         dq2 = (unsigned long long)__double2ll_rn((d2 - rint(d2)) * 18446744073709551616.0);
     }
     ts_block_scan2(dq1, dq2, scan_sm);  // exclusive prefix inside the chunk
-    if (tid == TS_CTL_IC) ts_publish(&agg_q[c], dq1, dq2, epoch);  // halo thread: sum over the chunk's own 127 ticks
+    if (tid == TS_CTL_IC) ts_publish(&agg_q[c], dq1, dq2, epoch);  // halo thread: sum over the chunk's own ticks
     ts_lookback(agg_q, c, epoch, lb_sm, err);
     __syncthreads();
     unsigned long long lbq1, lbq2;
@@ -559,7 +563,7 @@ size_t ts_control_agg_bytes(int B, int K) {
 cudaError_t ts_launch_setup(ts_voice *d_params, int sample, uint64_t seed, uint64_t g0, int B, int sr, int R, int64_t N, int K,
                             ts_voice_consts *vc, ts_vhdr *hdr, float *params_human, unsigned long long *d_active, int full,
                             cudaStream_t st) {
-    ts_setup_kernel<<<(unsigned)B, TS_CTL_THREADS, 0, st>>>(d_params, sample, seed, g0, B, sr, R, (long long)N, K, vc, hdr,
+    ts_setup_kernel<<<(unsigned)B, TS_SETUP_THREADS, 0, st>>>(d_params, sample, seed, g0, B, sr, R, (long long)N, K, vc, hdr,
                                                           params_human, d_active, full);
     return cudaGetLastError();
 }
