@@ -309,6 +309,7 @@ def run_ours(args, wl):
     # ---- roofline of the dominant kernel (audio): algorithmic bytes = 4 B per output sample
     rec = device_records(ts, W, wl, dev)
     roof = kernel_roofline(ts, wl, rec, audio_ring, sm_hz, 50)
+    two_ms = min(ts.ts_time_audio_two_streams(rec, sr, seconds, audio_ring, 50) for _ in range(3))
     fill_ms = ts.ts_time_fill(audio_ring, 5)
     fill_gbs = audio_ring.numel() * 4 / (fill_ms * 1e-3) / 1e9
     traffic = ncu_value("audio_kernel_traffic", wl.name)
@@ -320,6 +321,12 @@ def run_ours(args, wl):
                 "peak_source": roof["peak_source"], "algorithmic_bytes_per_launch": out_bytes,
                 "audio_kernel_ms": roof["audio_kernel_ms"], "control_kernel_ms": roof["control_kernel_ms"],
                 "timing": "CUDA events around 50 back-to-back launches of each kernel (ts_time_kernels); control = setup + control",
+                "audio_kernel_ms_two_streams": two_ms, "frac_two_streams": out_bytes / (two_ms * 1e-3) / 1e9 / roof["peak"],
+                "alu_frac_two_streams": roof["active_sample_fraction"] * B * N / (two_ms * 1e-3) / roof["alu_bound"]["peak"],
+                "audio_kernel_ms_two_streams_note": "interval / launches with the launches alternating between the two audio streams, as "
+                                                    "the streaming calls issue them: an inverse throughput (the ramp and drain of a launch are "
+                                                    "covered by the other stream), not the launch duration `frac` is computed from; "
+                                                    "frac_two_streams / alu_frac_two_streams are the two bounds on that basis",
                 "store_only_fill_gbs": fill_gbs,
                 "store_only_fill": f"{audio_ring.numel() * 4 >> 20} MiB of 128-bit zero stores, 5 launches (ts_time_fill): what a pure "
                                    "store stream reaches, beside the copy peak above",

@@ -193,6 +193,13 @@ int ts_last_kernel_ms(float host_ms[2]);
  * A batch that ts_render splits into several voice chunks is timed chunk by chunk and summed.  Synchronises. */
 int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, float *d_audio_ring, int n_ring, int reps,
                     float host_ms[2]);
+/* Measurement aid: the audio kernel as the streaming calls launch it -- `reps` launches alternating between the two
+ * low-priority audio streams, so that the ramp and drain of one launch (3.8 us for any kernel of this shape) are covered
+ * by the other stream's launch -- timed as one interval on the set stream.  *host_ms = interval / reps: an inverse
+ * throughput, NOT a launch duration (ts_time_kernels gives that); the difference is the part of a launch in which the SMs
+ * hold no CTA.  The batch must fit one voice chunk.  Synchronises. */
+int ts_time_audio_two_streams(const ts_voice *d_params, int B, int sr, double seconds, float *d_audio_ring, int n_ring,
+                              int reps, float *host_ms);
 /* Measurement aid: average device time of a store-only kernel (128-bit stores of zeros over d_dst[0 .. bytes)), `reps`
  * launches between one pair of CUDA events on the set stream -> *host_ms per launch.  What a pure store stream reaches on
  * this GPU, quoted beside the copy peak the roofline uses.  Synchronises. */

@@ -31,7 +31,7 @@ class _Out(C.Structure):
 EXPORTS = ["ts_sample_params", "ts_render", "ts_render_fmt", "ts_render_host", "ts_render_host_fmt", "ts_corpus_render",
            "ts_corpus_render_fmt", "ts_corpus_open", "ts_corpus_next", "ts_corpus_close", "ts_corpus_is_test", "ts_num_samples",
            "ts_num_ticks", "ts_num_ticks_r", "ts_set_stream", "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes",
-           "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_time_kernels", "ts_time_fill", "ts_time_alu_bound", "ts_time_pipes", "ts_last_kernel_ms",
+           "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_time_kernels", "ts_time_audio_two_streams", "ts_time_fill", "ts_time_alu_bound", "ts_time_pipes", "ts_last_kernel_ms",
            "ts_last_stats", "ts_render_r", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_debug_noise_u32", "ts_debug_controls",
            "ts_debug_phase"]
 TS_F32, TS_F16, TS_BF16 = 0, 1, 2
@@ -73,6 +73,7 @@ def lib():
     L.ts_num_ticks_r.argtypes = [C.c_int64, i32]
     L.ts_num_ticks_r.restype = C.c_int64
     L.ts_time_fill.argtypes = [vp, C.c_size_t, i32, vp]
+    L.ts_time_audio_two_streams.argtypes = [vp, i32, i32, f64, vp, i32, i32, vp]
     L.ts_time_alu_bound.argtypes = [i32, i32, vp]
     L.ts_time_pipes.argtypes = [vp]
     L.ts_render_controls_r.argtypes = [vp, i32, i32, f64, i32, vp]
@@ -188,6 +189,16 @@ def ts_time_kernels(params, sr: int, seconds: float, audio_ring, reps: int):
     _check(lib().ts_time_kernels(C.c_void_p(p.data_ptr()), p.shape[0], sr, float(seconds), C.c_void_p(audio_ring.data_ptr()),
                                  int(audio_ring.shape[0]), reps, ms))
     return float(ms[0]), float(ms[1])
+
+
+def ts_time_audio_two_streams(params, sr: int, seconds: float, audio_ring, reps: int) -> float:
+    """-> ms per audio launch when launches alternate between the two audio streams (inverse throughput, not a duration)."""
+    p = _dev_params(params)
+    ms = C.c_float()
+    _use_current_stream(p.device)
+    _check(lib().ts_time_audio_two_streams(C.c_void_p(p.data_ptr()), p.shape[0], sr, float(seconds), C.c_void_p(audio_ring.data_ptr()),
+                                           int(audio_ring.shape[0]), reps, C.byref(ms)))
+    return float(ms.value)
 
 
 def ts_last_stats():

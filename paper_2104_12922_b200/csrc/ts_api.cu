@@ -808,6 +808,56 @@ int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, flo
     return TS_OK;
 }
 
+int ts_time_audio_two_streams(const ts_voice *d_params, int B, int sr, double seconds, float *d_audio_ring, int n_ring, int reps,
+                              float *host_ms) {
+    if (!d_params || !d_audio_ring || !host_ms) return fail(TS_ENULL, "NULL argument%s");
+    if (n_ring <= 0 || reps <= 0) return fail(TS_EINVAL, "n_ring and reps must be positive%s");
+    int64_t N;
+    int K;
+    int rc = check_sizes(B, sr, seconds, &N, &K);
+    if (rc) return rc;
+    if (chunk_voices(B, K) < B) return fail(TS_EINVAL, "the batch must fit one voice chunk%s");
+    S.cur = &S.lane[0];
+    rc = prepare_common(sr);
+    if (rc) return rc;
+    rc = prepare_lane();
+    if (rc) return rc;
+    rc = ensure_streams();
+    if (rc) return rc;
+    const ws_layout_t L = ws_layout(B, K, true);
+    rc = ensure_ws(L, B, K);
+    if (rc) return rc;
+    ts_lane &ln = *S.cur;
+    char *ws = static_cast<char *>(ln.ws);
+    ts_tick *table = reinterpret_cast<ts_tick *>(ws);
+    ts_vhdr *hdr = reinterpret_cast<ts_vhdr *>(ws + L.off_hdr);
+    ts_voice_consts *vc = reinterpret_cast<ts_voice_consts *>(ws + L.off_vc);
+    for (auto &e : S.ev)
+        if (!e) TS_CUDA(cudaEventCreate(&e));
+    cudaStream_t st = ln.stream;
+    if (++ln.epoch == 0) {
+        TS_CUDA(cudaMemsetAsync(ws + L.off_agg, 0, L.agg_bytes, st));
+        ln.epoch = 1;
+    }
+    TS_CUDA(ts_launch_setup(const_cast<ts_voice *>(d_params), 0, 0, 0, B, sr, TS_R, N, K, vc, hdr, nullptr, nullptr, 0, st));
+    TS_CUDA(ts_launch_control(vc, B, sr, TS_R, N, K, table, ws + L.off_agg, ln.epoch, nullptr, 1, max_audible_samples(sr, N), ln.d_err, st));
+    TS_CUDA(cudaEventRecord(S.ev[0], st));
+    rc = fork_streams();
+    if (rc) return rc;
+    const int tails = tails_expected(seconds);
+    for (int r = 0; r < reps; ++r)  // the table is only read: launches on the two audio streams are independent
+        TS_CUDA(ts_launch_audio(table, hdr, B, N, K, d_audio_ring + (size_t)(r % n_ring) * (size_t)B * (size_t)N, TS_F32, 0, tails,
+                                max_audible_samples(sr, N), nullptr, S.lo[r & 1]));
+    rc = join_streams();
+    if (rc) return rc;
+    TS_CUDA(cudaEventRecord(S.ev[1], st));
+    TS_CUDA(cudaEventSynchronize(S.ev[1]));
+    float x = 0.f;
+    TS_CUDA(cudaEventElapsedTime(&x, S.ev[0], S.ev[1]));
+    *host_ms = x / (float)reps;
+    return TS_OK;
+}
+
 int ts_time_fill(void *d_dst, size_t bytes, int reps, float *host_ms) {
     if (!d_dst || !host_ms) return fail(TS_ENULL, "NULL argument%s");
     if (bytes < 16 || reps <= 0) return fail(TS_EINVAL, "bytes and reps must be positive%s");
