@@ -642,3 +642,57 @@ def test_audio_rate_control_mode_r1(T):
     assert_parity(g, o, "R=1 ragged")
     with pytest.raises(T.TsynthError):
         T.ts_render_r(d6, wl.sr, wl.seconds, 7)
+
+
+def test_iterator_multi_chunk_batches_odd_ring_fp16(T):
+    """1024-voice batches need several voice chunks (the control table is capped for L2) that alternate between the two
+    lanes, and an odd ring moves a slot from one audio stream to the other: the case the cross-stream ring events exist for.
+    Every batch handed out must equal ts_sample_params + ts_render_fmt bit for bit."""
+    import torch
+    T.ts_set_nebula(None)
+    B, sr, seconds, first = 1024, 44100, 4.0, 5                              # 4 chunks of 256 voices per batch
+    N = O.num_samples(sr, seconds)
+    assert T.ts_workspace_bytes(B, sr, seconds) < B * T.ts_num_ticks(N) * 80   # i.e. the table is chunked
+    pr = torch.zeros((3, B, 80), device="cuda")
+    ar = torch.full((3, B, N), 9.0, device="cuda", dtype=torch.float16)
+    T.ts_corpus_open(3, first, sr, seconds, T.TS_F16, pr, ar)
+    kept = {}
+    for k in range(6):
+        b = T.ts_corpus_next()
+        assert b["batch_index"] == first + k and b["slot"] == (first + k) % 3
+        assert b["is_test_first"] == O.corpus_is_test(b["first_voice"]) and b["is_test_last"] == O.corpus_is_test(b["first_voice"] + B - 1)
+        if k in (0, 4, 5):
+            kept[k] = (b["audio"].clone(), b["params"].clone())
+    T.ts_corpus_close()
+    torch.cuda.synchronize()
+    for k, (a, p) in kept.items():
+        q = T.ts_sample_params(3, first + k, B)
+        assert torch.equal(p.view(torch.int32), q.view(torch.int32)), k
+        assert torch.equal(a, T.ts_render_fmt(q, sr, seconds, T.TS_F16)), k
+    u, nk = O.sample_params(3, first + 5, B)
+    o = O.render_batch(u[:64], nk[:64], sr, N)
+    g = kept[5][0][:64].float().cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(g - o) <= MAX_ABS + 0.5 * ulp16(o, 10))
+
+
+def test_measurement_aids_are_sane(T):
+    """ts_time_pipes / ts_time_alu_bound / ts_time_fill / ts_time_audio_two_streams (bench.py's roofline inputs) run and
+    return values in the physically possible range of a B200."""
+    import torch
+    T.ts_set_nebula(None)
+    rates = T.ts_time_pipes()
+    assert len(rates) == 8 and all(0.9 < v < 20.0 for v in rates.values()), rates
+    assert rates["FFMA"] < rates["FFMA2"] < rates["MUFU.EX2"]                # packed fp32x2 is two cycles, MUFU eight
+    for fast in (True, False):
+        v = T.ts_time_alu_bound(fast, 16)
+        assert 1e11 < v < 3e12, v                                            # below 148 SMs x 128 lanes x 2 GHz / ~36 instr
+    buf = torch.empty(64 << 20, device="cuda", dtype=torch.uint8)
+    gbs = buf.numel() / (T.ts_time_fill(buf, 3) * 1e-3) / 1e9
+    assert 1000 < gbs < 9000, gbs
+    B, sr, seconds = 128, 44100, 4.0
+    p = T.ts_sample_params(0, 0, B)
+    ring = torch.empty((4, B, T.ts_num_samples(sr, seconds)), device="cuda")
+    ctl, aud = T.ts_time_kernels(p, sr, seconds, ring, 10)
+    two = T.ts_time_audio_two_streams(p, sr, seconds, ring, 10)
+    assert 0.005 < two <= aud * 1.05 and 0.005 < ctl < 0.2 and aud < 0.2, (ctl, aud, two)
+    assert torch.equal(ring[1], T.ts_render(p, sr, seconds))                 # the timing launches render the real thing
