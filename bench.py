@@ -218,7 +218,8 @@ def measure_config(ts, W, torch, name, dev, sm_hz):
     ts.ts_set_nebula(W.apply_nebula(ts.ts_default_nebula(), wl))
     out_bytes = B * N * 4
     nbuf = min(256, max(2, -(-(160 << 20) // out_bytes) + 1))
-    nbuf += nbuf & 1          # an even ring keeps every slot on one audio stream (no cross-stream events)
+    lanes = ts.ts_streaming_lanes()
+    nbuf += -nbuf % lanes     # a ring that is a multiple of the streaming lanes keeps every slot on one audio stream (no cross-stream events)
     audio_ring = torch.empty((nbuf, B, N), dtype=torch.float32, device=dev)
     rec = device_records(ts, W, wl, dev)
     steps = max(3, min(200, int(0.02 / (out_bytes / 2.0e12))))       # ~20 ms of device time per region
@@ -275,7 +276,8 @@ def run_ours(args, wl):
     # rotating output buffers: together larger than the 126 MB L2, so no step rewrites lines still cached
     out_bytes = B * N * 4
     nbuf = min(256, max(2, -(-(160 << 20) // out_bytes) + 1))
-    nbuf += nbuf & 1          # an even ring keeps every slot on one audio stream (no cross-stream events)
+    lanes = ts.ts_streaming_lanes()
+    nbuf += -nbuf % lanes     # a ring that is a multiple of the streaming lanes keeps every slot on one audio stream (no cross-stream events)
     audio_ring = torch.empty((nbuf, B, N), dtype=torch.float32, device=dev)
     params_ring = torch.empty((nbuf, B, 80), dtype=torch.float32, device=dev)
 
@@ -309,7 +311,10 @@ def run_ours(args, wl):
     # ---- roofline of the dominant kernel (audio): algorithmic bytes = 4 B per output sample
     rec = device_records(ts, W, wl, dev)
     roof = kernel_roofline(ts, wl, rec, audio_ring, sm_hz, 50)
-    two_ms = min(ts.ts_time_audio_two_streams(rec, sr, seconds, audio_ring, 50) for _ in range(3))
+    try:
+        two_ms = min(ts.ts_time_audio_two_streams(rec, sr, seconds, audio_ring, 50) for _ in range(3))
+    except ts.TsynthError:  # the batch needs several voice chunks (C3): the overlapped-launch figure is a one-chunk measurement
+        two_ms = None
     fill_ms = ts.ts_time_fill(audio_ring, 5)
     fill_gbs = audio_ring.numel() * 4 / (fill_ms * 1e-3) / 1e9
     traffic = ncu_value("audio_kernel_traffic", wl.name)
@@ -321,8 +326,9 @@ def run_ours(args, wl):
                 "peak_source": roof["peak_source"], "algorithmic_bytes_per_launch": out_bytes,
                 "audio_kernel_ms": roof["audio_kernel_ms"], "control_kernel_ms": roof["control_kernel_ms"],
                 "timing": "CUDA events around 50 back-to-back launches of each kernel (ts_time_kernels); control = setup + control",
-                "audio_kernel_ms_two_streams": two_ms, "frac_two_streams": out_bytes / (two_ms * 1e-3) / 1e9 / roof["peak"],
-                "alu_frac_two_streams": roof["active_sample_fraction"] * B * N / (two_ms * 1e-3) / roof["alu_bound"]["peak"],
+                "audio_kernel_ms_two_streams": two_ms,
+                "frac_two_streams": out_bytes / (two_ms * 1e-3) / 1e9 / roof["peak"] if two_ms else None,
+                "alu_frac_two_streams": roof["active_sample_fraction"] * B * N / (two_ms * 1e-3) / roof["alu_bound"]["peak"] if two_ms else None,
                 "audio_kernel_ms_two_streams_note": "interval / launches with the launches alternating between the two audio streams, as "
                                                     "the streaming calls issue them: an inverse throughput (the ramp and drain of a launch are "
                                                     "covered by the other stream), not the launch duration `frac` is computed from; "

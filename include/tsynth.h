@@ -96,8 +96,10 @@ int ts_render_host_fmt(uint64_t seed, uint64_t batch_index, int B, int sr, doubl
 /* Streaming corpus generation ("generated on the fly from a batch index"; BASELINE.json configs[2]):
  * batches first_batch .. first_batch + n_batches - 1 of B voices each, batch i sampled and rendered into ring slot
  * i % n_ring: records at d_params_ring[(i % n_ring) * B], audio at d_audio_ring[(i % n_ring) * B * N].  Same
- * results as n_batches calls of ts_sample_params + ts_render, but consecutive batches run on two internal streams
- * with a workspace each, so the control stage of one batch overlaps the audio stage of the previous one.  The
+ * results as n_batches calls of ts_sample_params + ts_render, but consecutive batches rotate over
+ * ts_streaming_lanes() internal lanes (a workspace, a high-priority setup / control stream and a low-priority audio
+ * stream each), so the control stage of one batch overlaps the audio stages of the previous ones.  n_ring a multiple
+ * of ts_streaming_lanes() keeps every ring slot on one audio stream (no cross-stream events are needed then).  The
  * work is ordered after everything queued on the set stream and the set stream continues after it; the call
  * itself does not synchronise.  A slot is overwritten n_ring batches later: consume it before that. */
 int ts_corpus_render(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds,
@@ -172,6 +174,7 @@ int ts_corpus_is_test(uint64_t g);
 /* D17: N = llround(sr*seconds);  S5: K = ceil(N/TS_R) + 1 control ticks. */
 int64_t ts_num_samples(int sr, double seconds);
 int64_t ts_num_ticks(int64_t N);
+int ts_streaming_lanes(void);                     /* lanes the streaming calls rotate batches over (3) */
 
 int ts_set_stream(void *cuda_stream);              /* cudaStream_t; NULL = legacy default stream   */
 int ts_default_nebula(ts_range host_out78[TS_NPARAM]); /* host copy of the built-in table S2        */
@@ -193,9 +196,10 @@ int ts_last_kernel_ms(float host_ms[2]);
  * A batch that ts_render splits into several voice chunks is timed chunk by chunk and summed.  Synchronises. */
 int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, float *d_audio_ring, int n_ring, int reps,
                     float host_ms[2]);
-/* Measurement aid: the audio kernel as the streaming calls launch it -- `reps` launches alternating between the two
- * low-priority audio streams, so that the ramp and drain of one launch (3.8 us for any kernel of this shape) are covered
- * by the other stream's launch -- timed as one interval on the set stream.  *host_ms = interval / reps: an inverse
+/* Measurement aid: the audio kernel as the streaming calls launch it -- `reps` launches rotating over the
+ * ts_streaming_lanes() low-priority audio streams (two in round 2, hence the name), so that the ramp and drain of one
+ * launch (3.8 us for any kernel of this shape) are covered by the other streams' launches -- timed as one interval on the
+ * set stream.  *host_ms = interval / reps: an inverse
  * throughput, NOT a launch duration (ts_time_kernels gives that); the difference is the part of a launch in which the SMs
  * hold no CTA.  The batch must fit one voice chunk.  Synchronises. */
 int ts_time_audio_two_streams(const ts_voice *d_params, int B, int sr, double seconds, float *d_audio_ring, int n_ring,

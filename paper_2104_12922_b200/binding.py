@@ -30,7 +30,7 @@ class _Out(C.Structure):
 
 EXPORTS = ["ts_sample_params", "ts_render", "ts_render_fmt", "ts_render_host", "ts_render_host_fmt", "ts_corpus_render",
            "ts_corpus_render_fmt", "ts_corpus_open", "ts_corpus_next", "ts_corpus_close", "ts_corpus_is_test", "ts_num_samples",
-           "ts_num_ticks", "ts_num_ticks_r", "ts_set_stream", "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes",
+           "ts_num_ticks", "ts_num_ticks_r", "ts_streaming_lanes", "ts_set_stream", "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes",
            "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_time_kernels", "ts_time_audio_two_streams", "ts_time_fill", "ts_time_alu_bound", "ts_time_pipes", "ts_last_kernel_ms",
            "ts_last_stats", "ts_render_r", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_debug_noise_u32", "ts_debug_controls",
            "ts_debug_phase"]
@@ -153,6 +153,10 @@ def ts_set_nebula(neb) -> None:
     if neb.shape != (NPARAM,):
         raise TsynthError("nebula must have 78 entries")
     _check(lib().ts_set_nebula(neb.ctypes.data_as(C.c_void_p)))
+
+
+def ts_streaming_lanes() -> int:
+    return lib().ts_streaming_lanes()
 
 
 def ts_workspace_bytes(B: int, sr: int, seconds: float) -> int:

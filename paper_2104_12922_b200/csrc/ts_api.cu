@@ -9,11 +9,11 @@
 
 namespace {
 
-// A lane = a workspace with the stream(s) that use it, so that two batches can be in flight at once.
-// Lane 0 serves ts_render / ts_render_host on the caller's stream.  Lanes 1 and 2 serve the streaming calls: they
-// share one HIGH-priority stream for the (latency-bound) setup and control kernels and one LOW-priority stream for
-// the (issue-bound) audio kernel, so that the control stage of batch i+1 is dispatched into the SMs while the audio
-// stage of batch i still runs and fills the issue slots it leaves idle.
+// A lane = a workspace with the stream(s) that use it, so that several batches can be in flight at once.
+// Lane 0 serves ts_render / ts_render_host on the caller's stream.  Lanes 1 .. TS_SL serve the streaming calls: each
+// has a HIGH-priority stream for the (latency-bound) setup and control kernels and a LOW-priority stream for the
+// (issue-bound) audio kernel, so that the control stage of batch i+1 is dispatched into the SMs while the audio
+// stages of batches i, i-1 still run and fills the issue slots they leave idle.
 struct ts_lane {
     cudaStream_t stream = nullptr;
     void *ws = nullptr;
@@ -25,12 +25,16 @@ struct ts_lane {
     unsigned long long *h_active = nullptr;  // pinned
     unsigned int *d_err = nullptr;           // raised by a kernel whose look-back wait gave up
     unsigned int *h_err = nullptr;           // pinned
-    // lanes 1, 2: the audio kernel goes to its own low-priority stream
+    // streaming lanes: the audio kernel goes to its own low-priority stream
     cudaStream_t audio_stream = nullptr;
     cudaEvent_t ctl_done = nullptr, aud_done = nullptr;
     bool aud_pending = false;  // aud_done was recorded after the latest audio kernel that reads this workspace
 };
-constexpr int TS_LANES = 3;
+#ifndef TS_SLANES
+#define TS_SLANES 3  // measured on C2: 2 lanes 32.3 us per step, 3 lanes 26.9, 4 lanes 27.1
+#endif
+constexpr int TS_SL = TS_SLANES;     // streaming lanes (each: a workspace, a high- and a low-priority stream)
+constexpr int TS_LANES = 1 + TS_SL;
 constexpr int TS_MAX_RING = 64;
 
 struct ts_corpus_state {  // the streaming iterator (ts_corpus_open / next / close)
@@ -53,9 +57,9 @@ struct ts_state {
     cudaEvent_t fork = nullptr;
     // the streaming calls' internal streams: one high-priority (setup, control) and one low-priority (audio) stream per
     // streaming lane, so that consecutive chunks overlap completely (kernel launch gaps included)
-    cudaStream_t hi[2] = {nullptr, nullptr}, lo[2] = {nullptr, nullptr};
-    cudaEvent_t batch_done[TS_MAX_RING][2] = {};  // audio of batch (count % TS_MAX_RING) issued on lo[x] has finished
-    cudaEvent_t join_ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaStream_t hi[TS_SL] = {}, lo[TS_SL] = {};
+    cudaEvent_t batch_done[TS_MAX_RING][TS_SL] = {};  // audio of batch (count % TS_MAX_RING) issued on lo[x] has finished
+    cudaEvent_t join_ev[2 * TS_SL] = {};
     // host staging for ts_render_host
     void *stage = nullptr;
     size_t stage_bytes = 0;
@@ -360,7 +364,7 @@ int ensure_streams() {
     if (S.fork) return TS_OK;
     int lo_p = 0, hi_p = 0;
     TS_CUDA(cudaDeviceGetStreamPriorityRange(&lo_p, &hi_p));  // numerically lower = higher priority
-    for (int x = 0; x < 2; ++x) {
+    for (int x = 0; x < TS_SL; ++x) {
         TS_CUDA(cudaStreamCreateWithPriority(&S.hi[x], cudaStreamNonBlocking, hi_p));
         TS_CUDA(cudaStreamCreateWithPriority(&S.lo[x], cudaStreamNonBlocking, lo_p));
         S.lane[1 + x].stream = S.hi[x];
@@ -378,17 +382,17 @@ int ensure_streams() {
 // All internal streams start after everything already queued on the caller's stream.
 int fork_streams() {
     TS_CUDA(cudaEventRecord(S.fork, S.lane[0].stream));
-    for (int x = 0; x < 2; ++x) {
+    for (int x = 0; x < TS_SL; ++x) {
         TS_CUDA(cudaStreamWaitEvent(S.hi[x], S.fork, 0));
         TS_CUDA(cudaStreamWaitEvent(S.lo[x], S.fork, 0));
     }
     return TS_OK;
 }
 
-// A batch on the internal streams (forked by the caller): the voice chunks of the batch alternate between the two
+// A batch on the internal streams (forked by the caller): the voice chunks of the batch rotate over the
 // streaming lanes, setup + control on `hi`, audio on `lo`, so that the control stage of one chunk overlaps the audio
 // stage of the previous one -- across the chunks of a batch as well as across batches.
-// seq: position of the batch in its sequence (chunk j of the batch runs on lane (seq + j) & 1).  n_ring > 0: the batch
+// seq: position of the batch in its sequence (chunk j of the batch runs on lane (seq + j) % TS_SL).  n_ring > 0: the batch
 // goes into the ring slot that batch seq - n_ring wrote: that batch's audio, possibly on the other audio stream, must
 // have finished first.
 int stream_batch(ts_voice *p, sample_spec smp, int B, int sr, double seconds, int fmt, void *a, float *params_human, uint64_t seq = 0,
@@ -398,15 +402,15 @@ int stream_batch(ts_voice *p, sample_spec smp, int B, int sr, double seconds, in
     int rc = check_sizes(B, sr, seconds, &N, &K);
     if (rc) return rc;
     const int Bc = chunk_voices(B, K);
-    // Single-chunk batches alternate strictly between the two lanes; with an even ring a slot is then always written
-    // on the same audio stream and stream order covers the hazard.
-    const bool same_stream = (Bc >= B) && (n_ring % 2 == 0);
+    // Single-chunk batches rotate strictly over the lanes; with a ring that is a multiple of TS_SL a slot is then always
+    // written on the same audio stream and stream order covers the hazard.
+    const bool same_stream = (Bc >= B) && (n_ring % TS_SL == 0);
     if (n_ring > 0 && !same_stream) {
         const uint64_t k = (uint64_t)(n_ring < TS_MAX_RING ? n_ring : TS_MAX_RING);
         if (seq >= k) {
             cudaEvent_t *ev = S.batch_done[(seq - k) % TS_MAX_RING];
-            for (int x = 0; x < 2; ++x)
-                for (int y = 0; y < 2; ++y) TS_CUDA(cudaStreamWaitEvent(S.lo[x], ev[y], 0));
+            for (int x = 0; x < TS_SL; ++x)
+                for (int y = 0; y < TS_SL; ++y) TS_CUDA(cudaStreamWaitEvent(S.lo[x], ev[y], 0));
         }
     }
     const size_t es = fmt_bytes(fmt);
@@ -415,7 +419,7 @@ int stream_batch(ts_voice *p, sample_spec smp, int B, int sr, double seconds, in
     int64_t launches = 0, chunks = 0;
     for (int b0 = 0; b0 < B && rc == TS_OK; b0 += Bc) {
         const int nb = (B - b0 < Bc) ? (B - b0) : Bc;
-        S.cur = &S.lane[1 + (int)((seq + (uint64_t)chunks) & 1)];
+        S.cur = &S.lane[1 + (int)((seq + (uint64_t)chunks) % (uint64_t)TS_SL)];
         rc = render_impl(p + b0, sample_spec{smp.on, smp.seed, smp.g0 + (uint64_t)b0}, nb, sr, seconds, fmt,
                          static_cast<char *>(a) + (size_t)b0 * (size_t)N * es,
                          params_human ? params_human + (size_t)b0 * TS_NPARAM : nullptr, 0, nullptr);
@@ -427,13 +431,13 @@ int stream_batch(ts_voice *p, sample_spec smp, int B, int sr, double seconds, in
     S.stats[0] = launches;
     S.stats[1] = chunks;
     if (rc == TS_OK && n_ring > 0 && !same_stream)
-        for (int x = 0; x < 2; ++x) TS_CUDA(cudaEventRecord(S.batch_done[seq % TS_MAX_RING][x], S.lo[x]));
+        for (int x = 0; x < TS_SL; ++x) TS_CUDA(cudaEventRecord(S.batch_done[seq % TS_MAX_RING][x], S.lo[x]));
     return rc;
 }
 
 // The caller's stream continues after all internal streams.
 int join_streams() {
-    for (int x = 0; x < 2; ++x) {
+    for (int x = 0; x < TS_SL; ++x) {
         TS_CUDA(cudaEventRecord(S.join_ev[2 * x], S.hi[x]));
         TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, S.join_ev[2 * x], 0));
         TS_CUDA(cudaEventRecord(S.join_ev[2 * x + 1], S.lo[x]));
@@ -452,13 +456,15 @@ int corpus_issue(uint64_t batch) {  // render `batch` into its slot and record t
                                 batch - C.first, C.cfg.n_ring);
     if (rc) return rc;
     // the slot is ready when the batch's audio on BOTH audio streams has finished
-    TS_CUDA(cudaEventRecord(S.join_ev[1], S.lo[1]));
-    TS_CUDA(cudaStreamWaitEvent(S.lo[0], S.join_ev[1], 0));
+    for (int x = 1; x < TS_SL; ++x) {
+        TS_CUDA(cudaEventRecord(S.join_ev[2 * x + 1], S.lo[x]));
+        TS_CUDA(cudaStreamWaitEvent(S.lo[0], S.join_ev[2 * x + 1], 0));
+    }
     TS_CUDA(cudaEventRecord(C.ready[slot], S.lo[0]));
     return TS_OK;
 }
 
-// A batch that needs several voice chunks (control table capped for L2) runs its chunks on the two internal lanes, so
+// A batch that needs several voice chunks (control table capped for L2) runs its chunks on the internal lanes, so
 // that setup + control of chunk k+1 overlap the audio kernel of chunk k; a single-chunk batch stays on the set stream.
 int render_audio(ts_voice *d_params, sample_spec smp, int B, int sr, double seconds, int fmt, void *d_audio, float *d_params_human) {
     int64_t N;
@@ -488,6 +494,7 @@ int ts_corpus_is_test(uint64_t g) { return (g / 1024u) % 10u == 9u; }
 
 int64_t ts_num_samples(int sr, double seconds) { return (int64_t)llround((double)sr * seconds); }
 int64_t ts_num_ticks(int64_t N) { return (N + TS_R - 1) / TS_R + 1; }
+int ts_streaming_lanes(void) { return TS_SL; }
 int64_t ts_num_ticks_r(int64_t N, int R) { return (R > 0) ? (N + R - 1) / R + 1 : 0; }
 
 int ts_sample_params(uint64_t seed, uint64_t batch_index, int B, ts_voice *d_params) {
@@ -621,7 +628,7 @@ int ts_corpus_next(ts_corpus_batch *host_out) {
     // slot not in flight: the batch n_ring - 1 ahead of the one handed out now goes into it, ordered after the caller's
     // stream (both internal streams wait for it).
     TS_CUDA(cudaEventRecord(C.consumed, S.lane[0].stream));
-    for (int x = 0; x < 2; ++x) {
+    for (int x = 0; x < TS_SL; ++x) {
         TS_CUDA(cudaStreamWaitEvent(S.lo[x], C.consumed, 0));
         TS_CUDA(cudaStreamWaitEvent(S.hi[x], C.consumed, 0));
     }
@@ -644,7 +651,7 @@ int ts_corpus_close(void) {
     ts_corpus_state &C = S.corpus;
     if (!C.open) return TS_OK;
     C.open = false;
-    for (int x = 0; x < 2; ++x) {
+    for (int x = 0; x < TS_SL; ++x) {
         TS_CUDA(cudaStreamSynchronize(S.hi[x]));
         TS_CUDA(cudaStreamSynchronize(S.lo[x]));
     }
@@ -729,7 +736,7 @@ void ts_shutdown(void) {
         L.stream = keep;
     }
     if (S.fork) { cudaEventDestroy(S.fork); S.fork = nullptr; }
-    for (int x = 0; x < 2; ++x) {
+    for (int x = 0; x < TS_SL; ++x) {
         if (S.hi[x]) { cudaStreamDestroy(S.hi[x]); S.hi[x] = nullptr; }
         if (S.lo[x]) { cudaStreamDestroy(S.lo[x]); S.lo[x] = nullptr; }
     }
@@ -845,9 +852,9 @@ int ts_time_audio_two_streams(const ts_voice *d_params, int B, int sr, double se
     rc = fork_streams();
     if (rc) return rc;
     const int tails = tails_expected(seconds);
-    for (int r = 0; r < reps; ++r)  // the table is only read: launches on the two audio streams are independent
+    for (int r = 0; r < reps; ++r)  // the table is only read: launches on the audio streams are independent
         TS_CUDA(ts_launch_audio(table, hdr, B, N, K, d_audio_ring + (size_t)(r % n_ring) * (size_t)B * (size_t)N, TS_F32, 0, tails,
-                                max_audible_samples(sr, N), nullptr, S.lo[r & 1]));
+                                max_audible_samples(sr, N), nullptr, S.lo[r % TS_SL]));
     rc = join_streams();
     if (rc) return rc;
     TS_CUDA(cudaEventRecord(S.ev[1], st));

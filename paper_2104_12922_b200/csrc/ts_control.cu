@@ -460,7 +460,8 @@ ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, 
 #pragma unroll
             for (int e = 0; e < 6; ++e) E[e] = Es[e][tid];
         }
-    } else {  // every lane (the warp votes on which powers are needed at all); dead lanes' values are unused
+    } else if (j0 + (tid & ~31) <= jsil) {  // warps with a live lane, every lane of them (the warp votes on which powers are
+                                            // needed at all; dead lanes' values are unused); unrolled: partial unrolling measured slower
 #pragma unroll
         for (int e = 0; e < 6; ++e) E[e] = ts_adsr_fast(tau, e, V, &MT);
     }
