@@ -211,7 +211,7 @@ int ts_time_fill(void *d_dst, size_t bytes, int reps, float *host_ms);
 /* Measurement aid: the ALU bound of the audible part, measured.  Runs the audio kernel's own sample loop (S9..S14: the
  * same device function, 20 samples per thread and pass, `reps` passes) with no control table, no global stores and no CTA
  * turnover at 8 warps per SM sub-partition, and returns the audible samples per second the SM pipes sustain with that
- * instruction mix (fastsin: the MUFU.SIN variant of the square/saw sine taken by voices with k <= 1024, else the
+ * instruction mix (fastsin: the MUFU.SIN variant of the square/saw sine taken by voices with k <= 512, else the
  * polynomial one).  Synchronises. */
 int ts_time_alu_bound(int fastsin, int reps, double *host_samples_per_s);
 /* Measurement aid: issue rate of the instruction kinds the audio kernel is made of, each alone, 8 warps per SM

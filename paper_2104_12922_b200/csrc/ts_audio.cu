@@ -80,11 +80,14 @@ template <int FMT> __device__ __forceinline__ uint32_t ts_cvt16(ts_f2 v) {
 constexpr float SIN_C3 = -0.16666659712791443f, SIN_C5 = 0.008333087898790836f, SIN_C7 = -0.00019811101083178073f,
                 SIN_C9 = 2.6089039693033556e-06f;
 // The 20 samples of one run (S9..S14) from its start state, into the thread's slice of the staging tile.
-// FASTSIN: the square/saw's sine through MUFU.SIN (absolute error 2^-21: 3.7e-7) instead of the relative-accuracy
-// polynomial.  The sine is multiplied by (pi/2) k before the tanh (S11), so this is only taken for voices whose
-// steepness k <= 1024 (note frequency above 10.9 Hz: 93 % of the voices under the default nebula): the error it adds
-// to a sample is then below (pi/2) 1024 * 3.7e-7 * 1.125 = 6.7e-4, a third of the 2e-3 bar, and only within ~1/k of a
-// cycle around the zero crossings (rel-RMS contribution < 3e-5) (H4; the flag is set by the setup kernel).
+// FASTSIN: the square/saw's sine through MUFU.SIN on the whole cycle instead of the relative-accuracy polynomial on the
+// nearest half cycle.  The sine is multiplied by (pi/2) k before the tanh (S11), so its ABSOLUTE error at the zero
+// crossings decides: near theta = +-pi the fp32 angle carries the rounding of the int -> float conversion, of the scaling
+// and of sin.approx's own multiplication by 1/(2 pi) (together <= 3.8e-7 rad) and MUFU.SIN adds 2^-21.4 (3.6e-7):
+// 7.4e-7.  Taken only for voices whose steepness k <= 512 (note frequency above 18.6 Hz: 89 % of the voices under the
+// default nebula): the error it adds to a sample is then below (pi/2) 512 * 7.4e-7 * 1.125 = 6.7e-4, a third of the 2e-3
+// bar, and only within ~1/k of a cycle around the zero crossings (rel-RMS contribution < 3e-5) (H4; the flag is set by
+// the setup kernel).
 template <int FMT, int FASTSIN>
 __device__ __forceinline__ void ts_render_run(double P1, double w1, const double e1a, double P2, double w2, const double e1b,
                                               float a1, float a2, float a3, const float da1, const float da2, const float da3,
@@ -94,6 +97,11 @@ __device__ __forceinline__ void ts_render_run(double P1, double w1, const double
         ts_f2 G1 = ts_pack(a1, a1 + da1), G2 = ts_pack(a2, a2 + da2), G3 = ts_pack(a3, a3 + da3);
         const ts_f2 DG1 = ts_dup(2.0f * da1), DG2 = ts_dup(2.0f * da2), DG3 = ts_dup(2.0f * da3);
         ulonglong2 *my2 = reinterpret_cast<ulonglong2 *>(my);
+        // S9 two samples at a time: the increments are geometric (w_{n+1} = rho w_n, rho = 1 + e1), so from (P_n, w_n)
+        //     P_{n+1} = P_n + w_n,   P_{n+2} = P_n + w_n (1 + rho),   w_{n+2} = w_n rho^2 = w_n + w_n (2 e1 + e1^2)
+        // three fp64 instructions per pair and oscillator instead of four
+        const double c2a = 2.0 + e1a, c2b = 2.0 + e1b;
+        const double e2a = fma(e1a, e1a, e1a + e1a), e2b = fma(e1b, e1b, e1b + e1b);
 #pragma unroll
         for (int g = 0; g < TS_RUN / 4; ++g) {
             uint32_t nz[4];
@@ -102,43 +110,49 @@ __device__ __forceinline__ void ts_render_run(double P1, double w1, const double
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 // ---- S9: phase accumulation for two consecutive samples (fp64, geometric increments)
-                const int xa = __double2loint(P1);
-                const int la = __double2loint(P2), ha = __double2hiint(P2);
-                P1 += w1; w1 = fma(w1, e1a, w1);
-                P2 += w2; w2 = fma(w2, e1b, w2);
-                const int xb = __double2loint(P1);
-                const int lb = __double2loint(P2), hb = __double2hiint(P2);
-                P1 += w1; w1 = fma(w1, e1a, w1);
-                P2 += w2; w2 = fma(w2, e1b, w2);
+                const double P1b = P1 + w1, P2b = P2 + w2;
+                const int xa = __double2loint(P1), xb = __double2loint(P1b);
+                const int la = __double2loint(P2), lb = __double2loint(P2b);
+                const int ha = __double2hiint(P2), hb = __double2hiint(P2b);
+                P1 = fma(w1, c2a, P1); w1 = fma(w1, e2a, w1);
+                P2 = fma(w2, c2b, P2); w2 = fma(w2, e2b, w2);
                 // ---- S10 sine VCO: frac(phi) is the signed Q0.32 in the low word
                 float r1a, r1b;
                 ts_unpack(ts_mul2(ts_pack((float)xa, (float)xb), ts_dup(1.4629180792671596e-9f)), r1a, r1b);  // 2 pi 2^-32
                 const ts_f2 Y1 = ts_pack(__sinf(r1a), __sinf(r1b));
-                // ---- S11 square/saw VCO: low word = signed Q0.32 of the nearest HALF cycle (H4); the parity of
-                // that half cycle (bit 0 of the high word, +1 if the low word is negative) is the sign sigma.
-                const uint32_t sa = (((uint32_t)la + ((uint32_t)ha << 31)) & 0x80000000u) | one_bits;
-                const uint32_t sb = (((uint32_t)lb + ((uint32_t)hb << 31)) & 0x80000000u) | one_bits;
-                const ts_f2 SIG = ts_pack(__uint_as_float(sa), __uint_as_float(sb));
-                const ts_f2 TH = ts_mul2(ts_pack((float)la, (float)lb), ts_dup(7.314590396335798e-10f));  // 2 pi 2^-33
+                // ---- S11 square/saw VCO
                 float ea, eb, da, db;
                 float tha, thb;
-                ts_unpack(TH, tha, thb);
-                ts_f2 SN;  // sin(th), th in [-pi/2, pi/2)
+                ts_f2 SN, SC;  // sin(theta) (up to the sign sigma), sigma + s cos(theta) (up to sigma)
                 if (FASTSIN) {
+                    // gentle voices (k <= TS_FASTSIN_K): the accumulator is biased like VCO 1's, its low word is the signed
+                    // Q0.32 of the whole cycle, and MUFU.SIN / MUFU.COS take theta in [-pi, pi) as it is: no half-cycle
+                    // parity, y2 = tanh(c sin theta) (1 + s cos theta) literally
+                    ts_unpack(ts_mul2(ts_pack((float)la, (float)lb), ts_dup(1.4629180792671596e-9f)), tha, thb);  // 2 pi 2^-32
                     SN = ts_pack(__sinf(tha), __sinf(thb));
+                    SC = ts_fma2(SHAPE, ts_pack(__cosf(tha), __cosf(thb)), ONE);
                 } else {
+                    // steep voices: low word = signed Q0.32 of the nearest HALF cycle (H4), so that theta -> 0 at BOTH zero
+                    // crossings of the sine and the polynomial's relative accuracy holds there; the parity of that half
+                    // cycle (bit 0 of the high word, +1 if the low word is negative) is the sign sigma, folded in as
+                    // y2 = sigma tanh (1 + s sigma cos) = tanh (sigma + s cos)
+                    const uint32_t sa = (((uint32_t)la + ((uint32_t)ha << 31)) & 0x80000000u) | one_bits;
+                    const uint32_t sb = (((uint32_t)lb + ((uint32_t)hb << 31)) & 0x80000000u) | one_bits;
+                    const ts_f2 SIG = ts_pack(__uint_as_float(sa), __uint_as_float(sb));
+                    const ts_f2 TH = ts_mul2(ts_pack((float)la, (float)lb), ts_dup(7.314590396335798e-10f));  // 2 pi 2^-33
+                    ts_unpack(TH, tha, thb);
                     const ts_f2 T2 = ts_mul2(TH, TH);
                     ts_f2 Q = ts_fma2(T2, ts_dup(SIN_C9), ts_dup(SIN_C7));
                     Q = ts_fma2(Q, T2, ts_dup(SIN_C5));
                     Q = ts_fma2(Q, T2, ts_dup(SIN_C3));
                     SN = ts_fma2(ts_mul2(TH, T2), Q, TH);
+                    SC = ts_fma2(SHAPE, ts_pack(__cosf(tha), __cosf(thb)), SIG);
                 }
-                const ts_f2 CS = ts_pack(__cosf(tha), __cosf(thb));
                 ts_unpack(ts_mul2(SN, TANH_C), ea, eb);
                 ts_unpack(ts_add2(ts_pack(ts_ex2(ea), ts_ex2(eb)), ONE), da, db);
-                // tanh((pi/2) k sin) = 1 - 2 / (1 + 2^(c sin));  y2 = sigma tanh (1 + s sigma cos) = tanh (sigma + s cos)
+                // tanh((pi/2) k sin) = 1 - 2 / (1 + 2^(c sin))
                 const ts_f2 TNH = ts_fma2(ts_pack(ts_rcp(da), ts_rcp(db)), ts_dup(-2.0f), ONE);
-                const ts_f2 Y2 = ts_mul2(TNH, ts_fma2(SHAPE, CS, SIG));
+                const ts_f2 Y2 = ts_mul2(TNH, SC);
                 // ---- S12 noise value (RZ conversion keeps the top 24 bits of x when x >= 2^31 and a few more
                 // below: within 2^-24 of (x >> 8) 2^-23 - 1), S13 VCAs, S14 mixer (gains carry the mixer levels)
                 const ts_f2 Z = ts_fma2(ts_pack(__uint2float_rz(nz[2 * h]), __uint2float_rz(nz[2 * h + 1])),
@@ -278,8 +292,8 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
         double P1 = p1 + MAGIC32, P2 = p2 + MAGIC33;
 
         if (MODE == 0) {
-            if (hd.pad[0])  // CTA-uniform: the voice's square/saw is gentle enough for MUFU.SIN
-                ts_render_run<FMT, 1>(P1, w1, e1a, P2, w2, e1b, a1, a2, a3, da1, da2, da3, blk0, hd.nk0, hd.nk1, hd.shape, hd.tanh_c,
+            if (hd.pad[0])  // CTA-uniform: the voice's square/saw is gentle enough for MUFU.SIN on the whole cycle
+                ts_render_run<FMT, 1>(P1, w1, e1a, p2 + MAGIC32, w2, e1b, a1, a2, a3, da1, da2, da3, blk0, hd.nk0, hd.nk1, hd.shape, hd.tanh_c,
                                       one_bits, my, my16);
             else
                 ts_render_run<FMT, 0>(P1, w1, e1a, P2, w2, e1b, a1, a2, a3, da1, da2, da3, blk0, hd.nk0, hd.nk1, hd.shape, hd.tanh_c,
@@ -378,7 +392,7 @@ ts_body_bench_kernel(float *__restrict__ sink, int reps, uint32_t nk0, uint32_t 
     uint2 *my16 = reinterpret_cast<uint2 *>(my);
     nk0 = __reduce_or_sync(0xffffffffu, nk0);  // warp-uniform for the compiler, as blockIdx-derived values are in the real kernel
     nk1 = __reduce_or_sync(0xffffffffu, nk1);
-    double P1 = MAGIC32 + 0.1 * threadIdx.x, P2 = MAGIC33 + 0.07 * threadIdx.x;
+    double P1 = MAGIC32 + 0.1 * threadIdx.x, P2 = (FASTSIN ? MAGIC32 : MAGIC33) + 0.07 * threadIdx.x;
     const double w1 = w0 * (1 + threadIdx.x), w2 = 1.3 * w0 * (1 + threadIdx.x);
 #pragma unroll 1
     for (int rep = 0; rep < reps; ++rep) {

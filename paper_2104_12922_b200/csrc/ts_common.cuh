@@ -33,7 +33,7 @@ struct __align__(16) ts_vhdr {
     uint32_t nk0, nk1;
     int32_t n_act;    // samples [n_act, N) are exactly 0 (multiple of TS_R, or N)
     int32_t n_ticks;  // table entries [0, n_ticks) are valid
-    int32_t pad[2];   // pad[0] != 0: steepness k <= 1024, the audio kernel may take the square/saw's sine from MUFU.SIN
+    int32_t pad[2];   // pad[0] != 0: steepness k <= 512, the audio kernel takes the square/saw from MUFU.SIN / MUFU.COS on the whole cycle
 };
 static_assert(sizeof(ts_vhdr) == 32, "ts_vhdr layout");
 

@@ -351,7 +351,7 @@ ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64
         const double fc = 440.0 * ts_exp2((h[0] + h[71] - 69.0) * (1.0 / 12.0), &MT);
         const double k = 12000.0 / (fc * (ts_log2(fc, &MT) * 0.30102999566398120));
         s_tanh_c = (float)(1.5707963267948966 * k * 2.0 * 1.4426950408889634);
-        s_fast = (k <= 1024.0) ? 1 : 0;
+        s_fast = (k <= 512.0) ? 1 : 0;  // ts_audio.cu: whole-cycle MUFU.SIN / MUFU.COS variant of the square/saw
     } else if (tid >= 96) {
         // The voice is silent for good once the release of all four audible envelopes is over (their
         // ramp is 1, so E = 0 exactly): adsr1, adsr2, lfo1_amp, lfo2_amp.  jsil = first tick with
