@@ -28,8 +28,18 @@ __device__ __forceinline__ float ts_rcp(float x) {
     return y;
 }
 
+// The output is written once and not read again by this path: its lines are marked evict-first in L2, so that 90 MB of
+// streaming stores per launch do not push the control table (read by every run, written by the control kernel just
+// before) and the other lanes' working sets out of the 126 MB L2.  Measured on C2: audio kernel 24.6 -> 22.6 us, the
+// same as with the silent tails not written at all.
+__device__ __forceinline__ unsigned long long ts_policy_evict_first() {
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
 __device__ __forceinline__ void ts_bulk_issue(void *gdst, uint32_t ssrc, uint32_t bytes) {  // TMA engine (UBLKCP)
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(ssrc), "r"(bytes)
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(gdst), "r"(ssrc), "r"(bytes),
+                 "l"(ts_policy_evict_first())
                  : "memory");
 }
 __device__ __forceinline__ void ts_bulk_store(void *gdst, const void *ssrc, uint32_t bytes) {
@@ -206,7 +216,7 @@ ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ h
     if (MODE == 0 && !TAIL && n_tile0 >= hd.n_act) {  // silent tile: exact zeros (S4 release over; pin P9)
         if (aligned) {
             float4 *r4 = reinterpret_cast<float4 *>(row);
-            for (int i = tid; i < count * ES / 16; i += TS_AUDIO_THREADS) r4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int i = tid; i < count * ES / 16; i += TS_AUDIO_THREADS) __stcs(&r4[i], make_float4(0.f, 0.f, 0.f, 0.f));  // streaming
         } else if (FMT == TS_F32) {
             for (int i = tid; i < count; i += TS_AUDIO_THREADS) reinterpret_cast<float *>(row)[i] = 0.f;
         } else {
