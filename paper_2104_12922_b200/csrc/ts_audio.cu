@@ -181,8 +181,11 @@ __device__ __forceinline__ void ts_render_run(double P1, double w1, const double
 // cvt.rn.{f16x2,bf16x2}.f32, on its way into the staging tile.
 // TPC: consecutive tiles of one voice rendered by one CTA, one after the other (large launches: halves the CTA turnover,
 // which costs ~14 % of an SM's time at one tile per CTA; small launches keep TPC = 1 so that the last wave stays short).
+#ifndef TS_AUDIO_MINB
+#define TS_AUDIO_MINB 10  // 48 registers: ten CTAs per SM (9 at 52 registers measured 2 % slower on C3, 11 CTAs with spills slower)
+#endif
 template <int MODE, int TAIL, int FMT, int TPC>
-__global__ void __launch_bounds__(TS_AUDIO_THREADS)
+__global__ void __launch_bounds__(TS_AUDIO_THREADS, TS_AUDIO_MINB)
 ts_audio_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict__ hdr, int B, int N, int K,
                 void *__restrict__ audio_, double *__restrict__ dbg_phase, int aligned, uint32_t one_bits, int swap) {
     __shared__ __align__(128) float4 stage[TS_TILE / 4];

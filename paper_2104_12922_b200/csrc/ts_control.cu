@@ -103,9 +103,10 @@ __device__ __forceinline__ double ts_adsr(double t, int e, const ts_voice_consts
 // x^a for x in [0,1], a > 0, without branches: exact 0 and 1 at the ends (S4 needs both: E = 0 exactly once the
 // release is over), clamped log2/exp2 in between.  Twelve of these per tick are independent chains, so the
 // fp64 latency that dominates this kernel overlaps instead of adding up.
+// x comes from ts_ramp_lin, i.e. it is already in [0, 1]; x = 0 needs no clamp either: ts_log2 works on the bit pattern and
+// returns about -1023 for it, the product is clamped to -1000 and the result is replaced by the exact 0 below.
 __device__ __forceinline__ double ts_pow01_sel(double x, double a, const ts_math_tables *T) {
-    const double xc = fmin(fmax(x, 1e-300), 1.0);
-    double p = ts_exp2(fmax(a * ts_log2(xc, T), -1000.0), T);
+    double p = ts_exp2(fmax(a * ts_log2(x, T), -1000.0), T);
     p = (x >= 1.0) ? 1.0 : p;
     return (x <= 0.0) ? 0.0 : p;
 }
@@ -408,7 +409,7 @@ template <int PHASES>
 __global__ void __launch_bounds__(TS_CTL_THREADS)
 ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, long long N, int K, int NC,
                   ts_tick *__restrict__ table, ts_agg *__restrict__ agg, unsigned int epoch, double *__restrict__ dbg_ctl,
-                  unsigned int *__restrict__ err, int swap) {
+                  unsigned int *__restrict__ err, int swap, long long J, double f0) {
     __shared__ ts_voice_consts V;
     __shared__ ts_math_tables MT;
     __shared__ unsigned long long scan_sm[64];
@@ -445,7 +446,7 @@ ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, 
         reinterpret_cast<uint4 *>(&V)[i] = __ldg(reinterpret_cast<const uint4 *>(vc + v) + i);
     __syncthreads();
     const double *h = V.h;
-    const long long J = (N + R - 1) / R;  // control intervals that hold samples (PHASES = 1: R == TS_R)
+    // J = ceil(N / R): control intervals that hold samples; f0 = 440 / sr: both divided once on the host
 
     // ================= phase 1: controls at tick j =================
     const int j = j0 + tid;
@@ -513,7 +514,6 @@ ts_control_kernel(const ts_voice_consts *__restrict__ vc, int B, int sr, int R, 
     double inc[2] = {0, 0}, e1[2] = {0, 0}, g20[2] = {TS_RUN, TS_RUN};
     if (act) {
         const double2 p0 = pitch[tid], p1 = pitch[tid + 1];
-        const double f0 = 440.0 / (double)sr;
 #pragma unroll 1
         for (int o = 0; o < 2; ++o) {
             const double pa = o ? p0.y : p0.x, pb = o ? p1.y : p1.x;
@@ -586,14 +586,16 @@ cudaError_t ts_launch_control(const ts_voice_consts *vc, int B, int sr, int R, i
     const int swap = NCL > 65535;
     const dim3 grid = swap ? dim3((unsigned)NCL, (unsigned)B) : dim3((unsigned)B, (unsigned)NCL);
     if (phases && R != TS_R && R != 1) return cudaErrorInvalidValue;  // the audio kernels are built on R = 100 and R = 1
+    const long long J64 = ((long long)N + R - 1) / R;
+    const double f0 = 440.0 / (double)sr;
     if (phases && R == 1)
         ts_control_kernel<2><<<grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
-                                                             static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err, swap);
+                                                             static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err, swap, J64, f0);
     else if (phases)
         ts_control_kernel<1><<<grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
-                                                                       static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err, swap);
+                                                                       static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err, swap, J64, f0);
     else
         ts_control_kernel<0><<<grid, TS_CTL_THREADS, 0, st>>>(vc, B, sr, R, (long long)N, K, NC, table,
-                                                                       static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err, swap);
+                                                                       static_cast<ts_agg *>(agg), epoch, dbg_ctl, d_err, swap, J64, f0);
     return cudaGetLastError();
 }
