@@ -296,12 +296,14 @@ def test_render_host_end_to_end(T):
 
 
 def test_corpus_render_matches_batch_by_batch(T):
-    """ts_corpus_render (two internal streams, ring of output slots) == ts_sample_params + ts_render, bitwise."""
+    """ts_corpus_render (ts_streaming_lanes() internal lanes, ring of output slots) == ts_sample_params + ts_render, bitwise.
+    Rings that are a multiple of the lane count keep a slot on one audio stream; the others need the cross-stream events."""
     import torch
     T.ts_set_nebula(None)
     B, sr, seconds, first = 5, 44100, 0.3, 7
     N = O.num_samples(sr, seconds)
-    for n_ring, n_batches in ((2, 2), (3, 7), (4, 9)):
+    assert T.ts_streaming_lanes() >= 2
+    for n_ring, n_batches in ((2, 2), (3, 7), (4, 9), (5, 12), (6, 14)):
         pr = torch.zeros((n_ring, B, 80), device="cuda")
         ar = torch.full((n_ring, B, N), 9.0, device="cuda")
         T.ts_corpus_render(3, first, n_batches, sr, seconds, pr, ar)
@@ -491,7 +493,7 @@ def test_corpus_iterator_hands_out_audio_params_and_split(T):
     T.ts_set_nebula(None)
     B, sr, seconds, first = 128, 44100, 0.25, 68
     N = O.num_samples(sr, seconds)
-    for n_ring in (2, 3):
+    for n_ring in (2, 3, 4):
         pr = torch.zeros((n_ring, B, 80), device="cuda")
         ar = torch.full((n_ring, B, N), 9.0, device="cuda")
         T.ts_corpus_open(0, first, sr, seconds, T.TS_F32, pr, ar)
