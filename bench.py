@@ -175,7 +175,7 @@ _ALU_PEAK = {}
 def alu_peak(ts):
     """Audible samples/s the SM pipes sustain on the audio kernel's own sample loop (ts_time_alu_bound: the same device
     function, no memory, no CTA turnover, 8 warps per sub-partition), measured once per process: MUFU.SIN variant of the
-    square/saw sine (taken by 93 % of the voices) and polynomial variant."""
+    square/saw sine (taken by 89 % of the voices) and polynomial variant."""
     if not _ALU_PEAK:
         _ALU_PEAK["fastsin"] = max(ts.ts_time_alu_bound(True, 64) for _ in range(3))
         _ALU_PEAK["poly"] = max(ts.ts_time_alu_bound(False, 64) for _ in range(3))
@@ -282,7 +282,7 @@ def run_ours(args, wl):
     params_ring = torch.empty((nbuf, B, 80), dtype=torch.float32, device=dev)
 
     # ---- the timed regions: K consecutive batch indices of this rank's contiguous range through the streaming call
-    # (sampler + setup + control + audio per batch, consecutive batches on two internal streams), R times
+    # (sampler + setup + control + audio per batch, consecutive batches on the internal streaming lanes), R times
     K, Wm, R = args.steps, args.warmup, args.repeats
     per_rank = Wm + K * R
     first, _count = shard.batch_range(rank, world, per_rank)
@@ -329,7 +329,7 @@ def run_ours(args, wl):
                 "audio_kernel_ms_two_streams": two_ms,
                 "frac_two_streams": out_bytes / (two_ms * 1e-3) / 1e9 / roof["peak"] if two_ms else None,
                 "alu_frac_two_streams": roof["active_sample_fraction"] * B * N / (two_ms * 1e-3) / roof["alu_bound"]["peak"] if two_ms else None,
-                "audio_kernel_ms_two_streams_note": "interval / launches with the launches alternating between the two audio streams, as "
+                "audio_kernel_ms_two_streams_note": "interval / launches with the launches rotating over the audio streams of the streaming lanes, as "
                                                     "the streaming calls issue them: an inverse throughput (the ramp and drain of a launch are "
                                                     "covered by the other stream), not the launch duration `frac` is computed from; "
                                                     "frac_two_streams / alu_frac_two_streams are the two bounds on that basis",

@@ -196,7 +196,7 @@ def ts_time_kernels(params, sr: int, seconds: float, audio_ring, reps: int):
 
 
 def ts_time_audio_two_streams(params, sr: int, seconds: float, audio_ring, reps: int) -> float:
-    """-> ms per audio launch when launches alternate between the two audio streams (inverse throughput, not a duration)."""
+    """-> ms per audio launch when launches rotate over the lanes' audio streams (inverse throughput, not a duration)."""
     p = _dev_params(params)
     ms = C.c_float()
     _use_current_stream(p.device)
