@@ -699,3 +699,50 @@ def test_measurement_aids_are_sane(T):
     two = T.ts_time_audio_two_streams(p, sr, seconds, ring, 10)
     assert 0.005 < two <= aud * 1.05 and 0.005 < ctl < 0.2 and aud < 0.2, (ctl, aud, two)
     assert torch.equal(ring[1], T.ts_render(p, sr, seconds))                 # the timing launches render the real thing
+
+
+# ---------------------------------------------------------------------------------- a randomised sweep at the bench's own shape
+def test_streamed_c2_batches_and_random_nebulae_every_voice(T):
+    """24 consecutive C2-sized batches through ts_corpus_render (the launch configuration bench.py times: three streaming
+    lanes, ring a multiple of the lanes) and 40 random nebulae at mixed sample rates / lengths, EVERY voice against the
+    oracle.  (A 58 880-voice run of the same sweep, 360 batches and 400 nebulae, had no failure: worst 7.0e-5 / 2.9e-6.)"""
+    import torch
+    T.ts_set_nebula(None)
+    B, sr, seconds = 128, 44100, 4.0
+    N = O.num_samples(sr, seconds)
+    n_ring = 2 * T.ts_streaming_lanes()
+    pr = torch.zeros((n_ring, B, 80), device="cuda")
+    ar = torch.zeros((n_ring, B, N), device="cuda")
+    worst = (0.0, 0.0, -1)
+    for start in range(2000, 2024, n_ring):
+        T.ts_corpus_render(5, start, n_ring, sr, seconds, pr, ar)
+        T.ts_sync()
+        for k in range(n_ring):
+            u, nk = O.sample_params(5, start + k, B)
+            assert np.array_equal(pr[k].cpu().numpy()[:, :78].view(np.uint32), u.view(np.uint32))
+            w = assert_parity(ar[k].cpu().numpy(), O.render_batch(u, nk, sr, N), f"streamed batch {start + k}")
+            worst = max(worst, w)
+    try:
+        for seed in range(100, 140):
+            rng = np.random.default_rng(seed)
+            neb_o = O.default_nebula()
+            lo, hi = neb_o["lo"].copy(), neb_o["hi"].copy()
+            a, b = rng.uniform(0, 0.4, 78), rng.uniform(0.6, 1.0, 78)
+            neb_o["lo"], neb_o["hi"] = lo + a * (hi - lo), lo + b * (hi - lo)
+            neb_o["curve"] = np.exp(rng.uniform(np.log(0.1), np.log(10.0), 78))
+            neb_o["symmetric"] = rng.integers(0, 2, 78)
+            neb_o["lo"][[6, 11, 16, 21, 26, 31]] = 0.1          # ADSR alpha stays positive (S4)
+            if seed % 3 == 0:
+                neb_o["hi"][1] = 4.0                            # long notes: few silent tails
+            neb_g = T.ts_default_nebula()
+            for f in ("lo", "hi", "curve", "symmetric"):
+                neb_g[f] = neb_o[f]
+            T.ts_set_nebula(neb_g)
+            Bq, srq, secq = 32, [44100, 48000, 22050, 96000][seed % 4], [1.3, 2.0, 0.777, 3.1][(seed // 4) % 4]
+            u, nk = O.sample_params(seed, 7, Bq)
+            g = T.ts_render(to_dev(u, nk), srq, secq)
+            w = assert_parity(g.cpu().numpy(), O.render_batch(u, nk, srq, O.num_samples(srq, secq), neb_o), f"nebula {seed}")
+            worst = max(worst, w)
+    finally:
+        T.ts_set_nebula(None)
+    print("sweep worst (max, relRMS, voice):", worst)
