@@ -109,6 +109,16 @@ int ts_corpus_render(uint64_t seed, uint64_t first_batch, int n_batches, int B, 
 int ts_corpus_render_fmt(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds, int fmt,
                          ts_voice *d_params_ring, void *d_audio_ring, int n_ring);
 
+/* Streaming with ONE NEBULA PER BATCH ("per-call tables per batch"; P:L145 a nebula is the table of
+ * (min, max, curve, symmetric) of all parameters; P:L270 the paper's tuning runs render 256 sounds under each of 1000
+ * candidate tables, curves log-uniform in [0.1, 10]).  As ts_corpus_render_fmt, but batch i is mapped with
+ * host_tables[i * TS_NPARAM .. (i + 1) * TS_NPARAM): same results as ts_set_nebula(table i) + ts_sample_params +
+ * ts_render per batch, with the batches overlapping on the streaming lanes.  All tables are checked first (TS_EINVAL as
+ * ts_set_nebula and ts_render would return, nothing launched) and uploaded once; host_tables may be freed when the call
+ * returns.  The active nebula (ts_set_nebula) is not changed by the call. */
+int ts_corpus_render_nebulae(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds, int fmt,
+                             const ts_range *host_tables, ts_voice *d_params_ring, void *d_audio_ring, int n_ring);
+
 /* Streaming corpus ITERATOR ("generated on the fly", P:L98 sounds paired with their
  * parameters, P:L102 train/test blocks).  ts_corpus_open() fixes the corpus (seed, B, sr, seconds, format), the caller's
  * ring of n_ring >= 2 output slots and the first batch index, and starts rendering n_ring - 1 batches ahead on the

@@ -29,7 +29,7 @@ class _Out(C.Structure):
 
 
 EXPORTS = ["ts_sample_params", "ts_render", "ts_render_fmt", "ts_render_host", "ts_render_host_fmt", "ts_corpus_render",
-           "ts_corpus_render_fmt", "ts_corpus_open", "ts_corpus_next", "ts_corpus_close", "ts_corpus_is_test", "ts_num_samples",
+           "ts_corpus_render_fmt", "ts_corpus_render_nebulae", "ts_corpus_open", "ts_corpus_next", "ts_corpus_close", "ts_corpus_is_test", "ts_num_samples",
            "ts_num_ticks", "ts_num_ticks_r", "ts_streaming_lanes", "ts_set_stream", "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes",
            "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_time_kernels", "ts_time_audio_two_streams", "ts_time_fill", "ts_time_alu_bound", "ts_time_pipes", "ts_last_kernel_ms",
            "ts_last_stats", "ts_render_r", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_debug_noise_u32", "ts_debug_controls",
@@ -68,6 +68,7 @@ def lib():
     L.ts_render_host_fmt.argtypes = [u64, u64, i32, i32, f64, i32, vp, vp]
     L.ts_corpus_render.argtypes = [u64, u64, i32, i32, i32, f64, vp, vp, i32]
     L.ts_corpus_render_fmt.argtypes = [u64, u64, i32, i32, i32, f64, i32, vp, vp, i32]
+    L.ts_corpus_render_nebulae.argtypes = [u64, u64, i32, i32, i32, f64, i32, vp, vp, vp, i32]
     L.ts_corpus_open.argtypes = [C.POINTER(_CorpusCfg), u64]
     L.ts_corpus_next.argtypes = [C.POINTER(_CorpusBatch)]
     L.ts_num_ticks_r.argtypes = [C.c_int64, i32]
@@ -322,6 +323,26 @@ def ts_corpus_render_fmt(seed: int, first_batch: int, n_batches: int, sr: int, s
     _use_current_stream(params_ring.device)
     _check(lib().ts_corpus_render_fmt(seed, first_batch, n_batches, B, sr, float(seconds), fmt, C.c_void_p(params_ring.data_ptr()),
                                       C.c_void_p(audio_ring.data_ptr()), R_))
+    return audio_ring
+
+
+def ts_corpus_render_nebulae(seed: int, first_batch: int, sr: int, seconds: float, fmt: int, nebulae, params_ring, audio_ring):
+    """One nebula per batch: nebulae is a sequence / array [n_batches, 78] of NEBULA_DTYPE; batch i of the stream is mapped
+    with table i.  audio_ring [R, B, N] in fmt, params_ring [R, B, 80] fp32."""
+    tabs = np.ascontiguousarray(nebulae, dtype=NEBULA_DTYPE)
+    if tabs.ndim != 2 or tabs.shape[1] != NPARAM or tabs.shape[0] < 1:
+        raise TsynthError("nebulae must be [n_batches, 78]")
+    R_, B = int(params_ring.shape[0]), int(params_ring.shape[1])
+    N = ts_num_samples(sr, seconds)
+    if not (params_ring.is_cuda and params_ring.is_contiguous() and params_ring.shape[2] == REC_FLOATS):
+        raise TsynthError("params_ring must be a contiguous CUDA float32 tensor [R, B, 80]")
+    if not (audio_ring.is_cuda and audio_ring.dtype == _fmt_dtype(fmt) and audio_ring.is_contiguous()
+            and tuple(audio_ring.shape) == (R_, B, N)):
+        raise TsynthError("audio_ring must be a contiguous CUDA tensor [R, B, N] of the chosen format")
+    _use_current_stream(params_ring.device)
+    _check(lib().ts_corpus_render_nebulae(seed, first_batch, int(tabs.shape[0]), B, sr, float(seconds), fmt,
+                                          tabs.ctypes.data_as(C.c_void_p), C.c_void_p(params_ring.data_ptr()),
+                                          C.c_void_p(audio_ring.data_ptr()), R_))
     return audio_ring
 
 

@@ -65,6 +65,11 @@ struct ts_state {
     size_t stage_bytes = 0;
     double *mmd_ws = nullptr;
     size_t mmd_ws_count = 0;
+    // per-batch nebulae of ts_corpus_render_nebulae: all tables of a call in the device layout, uploaded once
+    void *d_tables = nullptr, *h_tables = nullptr;  // h_tables: pinned
+    size_t tables_bytes = 0;
+    cudaEvent_t tables_up = nullptr;                // the upload of the latest call has executed
+    const void *batch_table = nullptr;              // the table of the batch being issued (NULL: the active nebula)
     // timing / stats
     bool timing = false;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
@@ -122,6 +127,19 @@ void default_nebula(ts_range *n) {  // table S2 (D6, D8); ranges from BASELINE.j
         set(b + 2, -0.5, 0.5, 1.0, 0);
     }
     for (int i = 74; i < 78; ++i) set(i, 0.0, 1.0, 1.0, 0);
+}
+
+int check_nebula(const ts_range *t) {
+    for (int i = 0; i < TS_NPARAM; ++i) {
+        const ts_range &r = t[i];
+        if (!(r.curve > 0.0) || !isfinite(r.lo) || !isfinite(r.hi) || !isfinite(r.curve))
+            return fail(TS_EINVAL, "nebula entries must be finite with curve > 0%s");
+        // weights (LFO shapes 35..39, 43..47; modulation mixer 48..67) are normalised by their sum: a negative
+        // range would make w / sum(w), and with it the pitch, unbounded
+        const bool weight = (i >= 35 && i <= 39) || (i >= 43 && i <= 47) || (i >= 48 && i <= 67);
+        if (weight && (r.lo < 0.0 || r.hi < 0.0)) return fail(TS_EINVAL, "nebula ranges of weights must not be negative%s");
+    }
+    return TS_OK;
 }
 
 void ensure_nebula() {
@@ -316,7 +334,8 @@ int render_impl(ts_voice *d_params, sample_spec smp, int B, int sr, double secon
         }
         TS_CUDA(ts_launch_setup(d_params + b0, smp.on ? 1 : 0, smp.seed, smp.g0 + (uint64_t)b0, nb, sr, R, N, K, vc, hdr,
                                 params_human ? params_human + (size_t)b0 * TS_NPARAM : nullptr,
-                                want_stats ? ln.d_active : nullptr, (mode == 1 || mode == 2 || mode == 3) ? 1 : 0, ln.stream));
+                                want_stats ? ln.d_active : nullptr, (mode == 1 || mode == 2 || mode == 3) ? 1 : 0, S.batch_table,
+                                ln.stream));
         TS_CUDA(ts_launch_control(vc, nb, sr, R, N, K, table, agg, ln.epoch,
                                   (mode == 3 || mode == 4) ? dbg + (size_t)b0 * 5 * K : nullptr, with_table ? 1 : 0,
                                   (mode == 0) ? max_audible_samples(sr, N) : (int64_t)-1, ln.d_err,
@@ -588,6 +607,74 @@ int ts_corpus_render(uint64_t seed, uint64_t first_batch, int n_batches, int B, 
     return ts_corpus_render_fmt(seed, first_batch, n_batches, B, sr, seconds, TS_F32, d_params_ring, d_audio_ring, n_ring);
 }
 
+int ts_corpus_render_nebulae(uint64_t seed, uint64_t first_batch, int n_batches, int B, int sr, double seconds, int fmt,
+                             const ts_range *host_tables, ts_voice *d_params_ring, void *d_audio_ring, int n_ring) {
+    if (!host_tables) return fail(TS_ENULL, "host_tables is NULL%s");
+    if (!d_params_ring || !d_audio_ring) return fail(TS_ENULL, "NULL ring%s");
+    if (n_batches <= 0 || n_ring <= 0) return fail(TS_EINVAL, "n_batches and n_ring must be positive%s");
+    if (S.corpus.open) return fail(TS_EINVAL, "a corpus iterator is open: close it first%s");
+    int64_t N;
+    int K;
+    int rc = check_sizes(B, sr, seconds, &N, &K);
+    if (rc) return rc;
+    if (!fmt_ok(fmt)) return fail(TS_EINVAL, "unknown output format%s");
+    ensure_nebula();
+    ts_range saved[TS_NPARAM];
+    memcpy(saved, S.nebula, sizeof saved);
+    // every table is checked before anything is launched (a refused table leaves nothing half rendered)
+    for (int i = 0; i < n_batches; ++i) {
+        rc = check_nebula(host_tables + (size_t)i * TS_NPARAM);
+        if (rc) return rc;
+        memcpy(S.nebula, host_tables + (size_t)i * TS_NPARAM, sizeof S.nebula);
+        const bool ok = nebula_supported(sr);
+        memcpy(S.nebula, saved, sizeof saved);
+        if (!ok) return fail(TS_EINVAL, "a table allows an oscillator increment above 2^18/R cycles per sample at this sr%s");
+    }
+    S.cur = &S.lane[0];
+    rc = prepare_common(sr);  // math tables (and the active nebula, if stale) go up on the caller's stream, before the fork
+    if (rc) return rc;
+    rc = ensure_streams();
+    if (rc) return rc;
+    // all tables of the call, in the device layout, in one upload on the caller's stream
+    const size_t tb = ts_nebula_device_bytes(), need = tb * (size_t)n_batches;
+    if (!S.tables_up) TS_CUDA(cudaEventCreateWithFlags(&S.tables_up, cudaEventDisableTiming));
+    else TS_CUDA(cudaEventSynchronize(S.tables_up));  // the previous call's upload has read the pinned staging buffer
+    if (need > S.tables_bytes) {
+        TS_CUDA(cudaStreamSynchronize(S.lane[0].stream));  // kernels of an earlier call may still read the old device copy
+        if (S.d_tables) cudaFree(S.d_tables);
+        if (S.h_tables) cudaFreeHost(S.h_tables);
+        S.d_tables = S.h_tables = nullptr;
+        S.tables_bytes = 0;
+        if (cudaMalloc(&S.d_tables, need) != cudaSuccess || cudaMallocHost(&S.h_tables, need) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(TS_ENOMEM, "allocation of the nebula tables failed%s");
+        }
+        S.tables_bytes = need;
+    }
+    for (int i = 0; i < n_batches; ++i)
+        ts_nebula_to_device_layout(host_tables + (size_t)i * TS_NPARAM, static_cast<char *>(S.h_tables) + tb * (size_t)i);
+    TS_CUDA(cudaMemcpyAsync(S.d_tables, S.h_tables, need, cudaMemcpyHostToDevice, S.lane[0].stream));
+    TS_CUDA(cudaEventRecord(S.tables_up, S.lane[0].stream));
+    rc = fork_streams();
+    if (rc) return rc;
+    const size_t es = fmt_bytes(fmt);
+    int64_t launches = 0;
+    for (int i = 0; i < n_batches && rc == TS_OK; ++i) {
+        const size_t slot = (size_t)(i % n_ring);
+        // the host-side decisions of a batch (silent-tail mode, launch extents) follow the batch's own table
+        memcpy(S.nebula, host_tables + (size_t)i * TS_NPARAM, sizeof S.nebula);
+        S.batch_table = static_cast<const char *>(S.d_tables) + tb * (size_t)i;
+        rc = stream_batch(d_params_ring + slot * (size_t)B, sample_spec{true, seed, (first_batch + (uint64_t)i) * (uint64_t)B}, B, sr,
+                          seconds, fmt, static_cast<char *>(d_audio_ring) + slot * (size_t)B * (size_t)N * es, nullptr, (uint64_t)i, n_ring);
+        launches += S.stats[0];
+    }
+    S.batch_table = nullptr;
+    memcpy(S.nebula, saved, sizeof saved);  // the active nebula is what it was
+    const int rj = join_streams();
+    S.stats[0] = launches;
+    return rc ? rc : rj;
+}
+
 int ts_corpus_open(const ts_corpus_cfg *host_cfg, uint64_t first_batch) {
     if (!host_cfg) return fail(TS_ENULL, "host_cfg is NULL%s");
     if (!host_cfg->d_audio_ring || !host_cfg->d_params_ring) return fail(TS_ENULL, "NULL ring%s");
@@ -673,15 +760,8 @@ int ts_set_nebula(const ts_range *host_in78) {
     if (!host_in78) {
         default_nebula(S.nebula);
     } else {
-        for (int i = 0; i < TS_NPARAM; ++i) {
-            const ts_range &r = host_in78[i];
-            if (!(r.curve > 0.0) || !isfinite(r.lo) || !isfinite(r.hi) || !isfinite(r.curve))
-                return fail(TS_EINVAL, "nebula entries must be finite with curve > 0%s");
-            // weights (LFO shapes 35..39, 43..47; modulation mixer 48..67) are normalised by their sum: a negative
-            // range would make w / sum(w), and with it the pitch, unbounded
-            const bool weight = (i >= 35 && i <= 39) || (i >= 43 && i <= 47) || (i >= 48 && i <= 67);
-            if (weight && (r.lo < 0.0 || r.hi < 0.0)) return fail(TS_EINVAL, "nebula ranges of weights must not be negative%s");
-        }
+        const int rc = check_nebula(host_in78);
+        if (rc) return rc;
         memcpy(S.nebula, host_in78, sizeof S.nebula);
     }
     S.nebula_init = true;
@@ -747,6 +827,13 @@ void ts_shutdown(void) {
             if (e) { cudaEventDestroy(e); e = nullptr; }
     if (S.stage) cudaFree(S.stage);
     if (S.mmd_ws) cudaFree(S.mmd_ws);
+    if (S.d_tables) cudaFree(S.d_tables);
+    if (S.h_tables) cudaFreeHost(S.h_tables);
+    if (S.tables_up) cudaEventDestroy(S.tables_up);
+    S.d_tables = S.h_tables = nullptr;
+    S.tables_bytes = 0;
+    S.tables_up = nullptr;
+    S.batch_table = nullptr;
     for (auto &e : S.ev)
         if (e) { cudaEventDestroy(e); e = nullptr; }
     S.stage = nullptr;
@@ -794,7 +881,7 @@ int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, flo
                 TS_CUDA(cudaMemsetAsync(agg, 0, L.agg_bytes, st));
                 ln.epoch = 1;
             }
-            TS_CUDA(ts_launch_setup(const_cast<ts_voice *>(d_params) + b0, 0, 0, 0, nb, sr, TS_R, N, K, vc, hdr, nullptr, nullptr, 0, st));
+            TS_CUDA(ts_launch_setup(const_cast<ts_voice *>(d_params) + b0, 0, 0, 0, nb, sr, TS_R, N, K, vc, hdr, nullptr, nullptr, 0, nullptr, st));
             TS_CUDA(ts_launch_control(vc, nb, sr, TS_R, N, K, table, agg, ln.epoch, nullptr, 1, max_audible_samples(sr, N), ln.d_err, st));
         }
         TS_CUDA(cudaEventRecord(S.ev[1], st));
@@ -846,7 +933,7 @@ int ts_time_audio_two_streams(const ts_voice *d_params, int B, int sr, double se
         TS_CUDA(cudaMemsetAsync(ws + L.off_agg, 0, L.agg_bytes, st));
         ln.epoch = 1;
     }
-    TS_CUDA(ts_launch_setup(const_cast<ts_voice *>(d_params), 0, 0, 0, B, sr, TS_R, N, K, vc, hdr, nullptr, nullptr, 0, st));
+    TS_CUDA(ts_launch_setup(const_cast<ts_voice *>(d_params), 0, 0, 0, B, sr, TS_R, N, K, vc, hdr, nullptr, nullptr, 0, nullptr, st));
     TS_CUDA(ts_launch_control(vc, B, sr, TS_R, N, K, table, ws + L.off_agg, ln.epoch, nullptr, 1, max_audible_samples(sr, N), ln.d_err, st));
     TS_CUDA(cudaEventRecord(S.ev[0], st));
     rc = fork_streams();

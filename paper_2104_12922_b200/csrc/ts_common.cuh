@@ -93,7 +93,9 @@ size_t ts_mmd_partial_count(int n);
 // R: samples per control tick (TS_R on the audio path; any R >= 1 for control-rate rendering on its own)
 cudaError_t ts_launch_setup(ts_voice *d_params, int sample, uint64_t seed, uint64_t g0, int B, int sr, int R, int64_t N, int K,
                             ts_voice_consts *vc, ts_vhdr *hdr, float *params_human, unsigned long long *d_active, int full,
-                            cudaStream_t st);
+                            const void *d_nebula, cudaStream_t st);  // d_nebula: a table in the device layout, NULL = the active nebula
+size_t ts_nebula_device_bytes();                                           // bytes of one table in the device layout
+void ts_nebula_to_device_layout(const ts_range *host78, void *out);       // host-side conversion (adds 1 / curve)
 // phases != 0: also the S9 tick-level phase scan and the control table (needed by the audio kernel); phases == 0 stops
 // after the modulation mixer (control-rate rendering on its own).  n_audible_max >= 0: no voice is audible at or after this sample (chunks past it are not launched); d_err: device flag raised if a look-back wait gives up
 cudaError_t ts_launch_control(const ts_voice_consts *vc, int B, int sr, int R, int64_t N, int K, ts_tick *table, void *agg,

@@ -30,9 +30,14 @@ __device__ ts_math_tables c_math;
 
 cudaError_t ts_upload_nebula(const ts_range *host78, cudaStream_t st) {
     static ts_range_dev D[TS_NPARAM];  // static: the async copy reads it after this function returns
+    ts_nebula_to_device_layout(host78, D);
+    return cudaMemcpyToSymbolAsync(c_nebula, D, sizeof D, 0, cudaMemcpyHostToDevice, st);
+}
+size_t ts_nebula_device_bytes() { return sizeof(ts_range_dev) * TS_NPARAM; }
+void ts_nebula_to_device_layout(const ts_range *host78, void *out) {
+    ts_range_dev *D = static_cast<ts_range_dev *>(out);
     for (int i = 0; i < TS_NPARAM; ++i)
         D[i] = ts_range_dev{host78[i].lo, host78[i].hi, host78[i].curve, 1.0 / host78[i].curve, (long long)host78[i].symmetric};
-    return cudaMemcpyToSymbolAsync(c_nebula, D, sizeof D, 0, cudaMemcpyHostToDevice, st);
 }
 
 cudaError_t ts_upload_math_tables(cudaStream_t st) {
@@ -278,7 +283,8 @@ __device__ __forceinline__ double ts_lfo_mix(double p, const double *wn) {
 __global__ void __launch_bounds__(TS_SETUP_THREADS)
 ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64_t g0, int B, int sr, int R, long long N, int K,
                 ts_voice_consts *__restrict__ vc, ts_vhdr *__restrict__ hdr, float *__restrict__ params_human,
-                unsigned long long *__restrict__ d_active, int full) {
+                unsigned long long *__restrict__ d_active, int full, const ts_range_dev *__restrict__ neb_table) {
+    const ts_range_dev *neb = neb_table ? neb_table : c_nebula;  // a table of this launch's own (per-batch nebulae) or the active one
     __shared__ ts_voice_consts V;
     __shared__ ts_math_tables MT;
     __shared__ __align__(16) float su[TS_NPARAM + 2];
@@ -314,7 +320,7 @@ ts_setup_kernel(ts_voice *__restrict__ params, int sample, uint64_t seed, uint64
         __syncthreads();
     }
     if (tid < TS_NPARAM) {
-        const double hv = ts_map((double)su[tid], c_nebula[tid], &MT);
+        const double hv = ts_map((double)su[tid], neb[tid], &MT);
         V.h[tid] = hv;
         if (params_human) params_human[(size_t)v * TS_NPARAM + tid] = (float)hv;
     }
@@ -563,9 +569,9 @@ size_t ts_control_agg_bytes(int B, int K) {
 
 cudaError_t ts_launch_setup(ts_voice *d_params, int sample, uint64_t seed, uint64_t g0, int B, int sr, int R, int64_t N, int K,
                             ts_voice_consts *vc, ts_vhdr *hdr, float *params_human, unsigned long long *d_active, int full,
-                            cudaStream_t st) {
+                            const void *d_nebula, cudaStream_t st) {
     ts_setup_kernel<<<(unsigned)B, TS_SETUP_THREADS, 0, st>>>(d_params, sample, seed, g0, B, sr, R, (long long)N, K, vc, hdr,
-                                                          params_human, d_active, full);
+                                                          params_human, d_active, full, static_cast<const ts_range_dev *>(d_nebula));
     return cudaGetLastError();
 }
 

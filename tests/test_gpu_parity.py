@@ -746,3 +746,57 @@ def test_streamed_c2_batches_and_random_nebulae_every_voice(T):
     finally:
         T.ts_set_nebula(None)
     print("sweep worst (max, relRMS, voice):", worst)
+
+
+# ---------------------------------------------------------------------------------- one nebula per batch
+def _random_nebula(seed):
+    rng = np.random.default_rng(seed)
+    neb = O.default_nebula()
+    lo, hi = neb["lo"].copy(), neb["hi"].copy()
+    a, b = rng.uniform(0, 0.4, 78), rng.uniform(0.6, 1.0, 78)
+    neb["lo"], neb["hi"] = lo + a * (hi - lo), lo + b * (hi - lo)
+    neb["curve"] = np.exp(rng.uniform(np.log(0.1), np.log(10.0), 78))
+    neb["symmetric"] = rng.integers(0, 2, 78)
+    neb["lo"][[6, 11, 16, 21, 26, 31]] = 0.1                            # ADSR alpha stays positive (S4)
+    if seed % 2:
+        neb["hi"][1] = 3.0                                              # long notes: the other silent-tail mode
+    return neb
+
+
+def test_corpus_render_with_one_nebula_per_batch(T):
+    """ts_corpus_render_nebulae: batch i under table i == ts_set_nebula(table i) + ts_sample_params + ts_render, bitwise;
+    every voice against the oracle under its batch's table; the active nebula is untouched; a bad table refuses the call."""
+    import torch
+    T.ts_set_nebula(None)
+    B, sr, seconds, first, nb = 16, 44100, 4.0, 40, 7          # 4 s: odd batches (3 s notes) take TAIL = 0, even ones TAIL = 1
+    N = O.num_samples(sr, seconds)
+    nebs_o = [_random_nebula(300 + i) for i in range(nb)]
+    tabs = np.zeros((nb, 78), dtype=T.NEBULA_DTYPE)
+    for i, n in enumerate(nebs_o):
+        for f in ("lo", "hi", "curve", "symmetric"):
+            tabs[i][f] = n[f]
+    for n_ring in (T.ts_streaming_lanes(), 4):
+        pr = torch.zeros((n_ring, B, 80), device="cuda")
+        ar = torch.full((n_ring, B, N), 9.0, device="cuda")
+        T.ts_corpus_render_nebulae(11, first, sr, seconds, T.TS_F32, tabs, pr, ar)
+        T.ts_sync()
+        got = {i % n_ring: i for i in range(nb)}                         # slot -> last batch written to it
+        for slot, i in got.items():
+            u, nk = O.sample_params(11, first + i, B)
+            assert np.array_equal(pr[slot].cpu().numpy()[:, :78].view(np.uint32), u.view(np.uint32))
+            assert_parity(ar[slot].cpu().numpy(), O.render_batch(u, nk, sr, N, nebs_o[i]), f"nebula of batch {i}")
+            T.ts_set_nebula(tabs[i])
+            assert torch.equal(ar[slot], T.ts_render(T.ts_sample_params(11, first + i, B), sr, seconds)), (n_ring, slot, i)
+            T.ts_set_nebula(None)
+        # the call left the active (default) nebula alone
+        u, nk = O.sample_params(11, first, B)
+        assert_parity(T.ts_render(to_dev(u, nk), sr, seconds).cpu().numpy(), O.render_batch(u, nk, sr, N), "active nebula")
+    bad = tabs.copy()
+    bad[3]["curve"][5] = -1.0
+    with pytest.raises(T.TsynthError):
+        T.ts_corpus_render_nebulae(11, first, sr, seconds, T.TS_F32, bad, pr, ar)
+    bad = tabs.copy()
+    bad[2]["hi"][0] = 400.0                                             # pitch beyond the supported increment (D23)
+    with pytest.raises(T.TsynthError):
+        T.ts_corpus_render_nebulae(11, first, sr, seconds, T.TS_F32, bad, pr, ar)
+    T.ts_sync()
