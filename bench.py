@@ -412,6 +412,27 @@ def run_ours(args, wl):
                           "peak_s": alu_s, "frac": alu_s / (mmd_ms * 1e-3),
                           "what": "Eq. 2 with the l1 core distance (P:L230); bound = 2 FADD-class instructions per (pair, component) "
                                   "at 148 SMs x 128 fp32 lanes per clock; embeddings (4 MB) are L2-resident"}
+        # ---- a nebula sweep in the shape of the paper's tuning runs (256 sounds per candidate table)
+        import numpy as np
+        nt, Bn = 24, 256
+        rng = np.random.default_rng(0)
+        tabs = np.stack([ts.ts_default_nebula() for _ in range(nt)])
+        for t in tabs:
+            t["curve"] = np.exp(rng.uniform(np.log(0.1), np.log(10.0), t.shape[0]))   # log-uniform in [0.1, 10]
+        lanes = ts.ts_streaming_lanes()
+        prn = torch.empty((lanes, Bn, 80), dtype=torch.float32, device=dev)
+        arn = torch.empty((lanes, Bn, N), dtype=torch.float32, device=dev)
+        ts.ts_corpus_render_nebulae(wl.seed, 0, sr, seconds, ts.TS_F32, tabs, prn, arn)
+        torch.cuda.synchronize()
+        e0.record()
+        ts.ts_corpus_render_nebulae(wl.seed, nt, sr, seconds, ts.TS_F32, tabs, prn, arn)
+        e1.record()
+        torch.cuda.synchronize()
+        sweep_ms = e0.elapsed_time(e1)
+        line["nebula_sweep"] = {"ms_per_table": sweep_ms / nt, "samples_per_s": nt * Bn * N / (sweep_ms * 1e-3), "tables": nt,
+                                "voices_per_table": Bn, "what": "ts_corpus_render_nebulae: one candidate table (curves log-uniform in "
+                                "[0.1, 10], P:L270) per batch of 256 voices x 4 s, table upload included"}
+        del prn, arn
         if not args.no_cpu_baseline:
             cores = os.cpu_count() or 1
             voices = min(wl.B, 128)
