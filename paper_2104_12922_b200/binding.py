@@ -32,7 +32,7 @@ EXPORTS = ["ts_sample_params", "ts_render", "ts_render_fmt", "ts_render_host", "
            "ts_corpus_render_fmt", "ts_corpus_render_nebulae", "ts_corpus_open", "ts_corpus_next", "ts_corpus_close", "ts_corpus_is_test", "ts_num_samples",
            "ts_num_ticks", "ts_num_ticks_r", "ts_streaming_lanes", "ts_set_stream", "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes",
            "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_time_kernels", "ts_time_audio_two_streams", "ts_time_fill", "ts_time_alu_bound", "ts_time_pipes", "ts_last_kernel_ms",
-           "ts_last_stats", "ts_render_r", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_debug_noise_u32", "ts_debug_controls",
+           "ts_last_stats", "ts_render_r", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_mmd_l1_pairwise", "ts_mmd_l1_sorted", "ts_debug_noise_u32", "ts_debug_controls",
            "ts_debug_phase"]
 TS_F32, TS_F16, TS_BF16 = 0, 1, 2
 
@@ -80,6 +80,8 @@ def lib():
     L.ts_render_controls_r.argtypes = [vp, i32, i32, f64, i32, vp]
     L.ts_render_r.argtypes = [vp, i32, i32, f64, i32, vp]
     L.ts_mmd_l1.argtypes = [vp, vp, i32, i32, vp]
+    L.ts_mmd_l1_pairwise.argtypes = [vp, vp, i32, i32, vp]
+    L.ts_mmd_l1_sorted.argtypes = [vp, vp, i32, i32, vp]
     L.ts_corpus_is_test.argtypes = [u64]
     L.ts_num_samples.argtypes = [i32, f64]
     L.ts_num_samples.restype = C.c_int64
@@ -437,15 +439,17 @@ def ts_render_controls_r(params, sr: int, seconds: float, R: int):
     return out
 
 
-def ts_mmd_l1(x, y):
-    """x, y: CUDA float32 [n, d] -> CUDA float64 [4]: MMD (Eq. 2), sum |x_i - y_j|_1, sum |x_i - x_j|_1, sum |y_i - y_j|_1."""
+def ts_mmd_l1(x, y, form: str = "auto"):
+    """x, y: CUDA float32 [n, d] -> CUDA float64 [4]: MMD (Eq. 2), sum |x_i - y_j|_1, sum |x_i - x_j|_1, sum |y_i - y_j|_1.
+    form: "auto" (ts_mmd_l1: the faster form at this n), "pairwise" (ts_mmd_l1_pairwise) or "sorted" (ts_mmd_l1_sorted)."""
     torch = _torch()
     if not (x.is_cuda and y.is_cuda and x.dtype == torch.float32 and y.dtype == torch.float32 and x.is_contiguous()
             and y.is_contiguous() and x.dim() == 2 and tuple(x.shape) == tuple(y.shape)):
         raise TsynthError("x and y must be contiguous CUDA float32 tensors of the same shape [n, d]")
     out = torch.empty(4, dtype=torch.float64, device=x.device)
     _use_current_stream(x.device)
-    _check(lib().ts_mmd_l1(C.c_void_p(x.data_ptr()), C.c_void_p(y.data_ptr()), int(x.shape[0]), int(x.shape[1]), C.c_void_p(out.data_ptr())))
+    fn = {"auto": lib().ts_mmd_l1, "pairwise": lib().ts_mmd_l1_pairwise, "sorted": lib().ts_mmd_l1_sorted}[form]
+    _check(fn(C.c_void_p(x.data_ptr()), C.c_void_p(y.data_ptr()), int(x.shape[0]), int(x.shape[1]), C.c_void_p(out.data_ptr())))
     return out
 
 

@@ -1032,12 +1032,15 @@ int ts_render_controls(const ts_voice *d_params, int B, int sr, double seconds, 
     return ts_render_controls_r(d_params, B, sr, seconds, TS_R, d_ctl);
 }
 
-int ts_mmd_l1(const float *d_x, const float *d_y, int n, int d, double *d_out) {
+static int mmd_impl(const float *d_x, const float *d_y, int n, int d, double *d_out, int pairwise) {
     if (!d_x || !d_y || !d_out) return fail(TS_ENULL, "NULL argument%s");
     if (n <= 0 || d <= 0 || n > 65535) return fail(TS_EINVAL, "n must be in [1, 65535] and d positive%s");
-    const size_t need = ts_mmd_partial_count(n);
+    const size_t need = ts_mmd_partial_count(n, d);
     if (need > S.mmd_ws_count) {
-        if (S.mmd_ws) cudaFree(S.mmd_ws);
+        if (S.mmd_ws) {
+            cudaStreamSynchronize(S.lane[0].stream);  // an earlier call may still use the old workspace
+            cudaFree(S.mmd_ws);
+        }
         S.mmd_ws = nullptr;
         S.mmd_ws_count = 0;
         if (cudaMalloc(&S.mmd_ws, need * sizeof(double)) != cudaSuccess) {
@@ -1046,9 +1049,12 @@ int ts_mmd_l1(const float *d_x, const float *d_y, int n, int d, double *d_out) {
         }
         S.mmd_ws_count = need;
     }
-    TS_CUDA(ts_launch_mmd(d_x, d_y, n, d, S.mmd_ws, d_out, S.lane[0].stream));
+    TS_CUDA(ts_launch_mmd(d_x, d_y, n, d, S.mmd_ws, d_out, pairwise, S.lane[0].stream));
     return TS_OK;
 }
+int ts_mmd_l1(const float *d_x, const float *d_y, int n, int d, double *d_out) { return mmd_impl(d_x, d_y, n, d, d_out, 0); }
+int ts_mmd_l1_pairwise(const float *d_x, const float *d_y, int n, int d, double *d_out) { return mmd_impl(d_x, d_y, n, d, d_out, 1); }
+int ts_mmd_l1_sorted(const float *d_x, const float *d_y, int n, int d, double *d_out) { return mmd_impl(d_x, d_y, n, d, d_out, 2); }
 
 int ts_debug_noise_u32(const uint32_t host_key[2], uint64_t n0, int count, uint32_t *d_out) {
     if (!host_key || !d_out) return fail(TS_ENULL, "NULL argument%s");

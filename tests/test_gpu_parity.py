@@ -518,25 +518,54 @@ def test_corpus_iterator_hands_out_audio_params_and_split(T):
 
 
 # ---------------------------------------------------------------------------------- Eq. 2: MMD with the l1 core distance
-@pytest.mark.parametrize("n,d", [(1000, 512), (37, 5), (64, 32), (129, 100), (1, 3)])
+@pytest.mark.parametrize("n,d", [(1000, 512), (37, 5), (64, 32), (129, 100), (1, 3), (256, 7), (257, 2), (3000, 16)])
 def test_mmd_l1_against_oracle(T, n, d):
-    """The paper's setting (n = 1000 sounds, d = 512 OpenL3 values) and ragged sizes.  Differences and per-pair
-    sums are fp32 on the GPU (inputs O(1): each |x - y| carries 2^-24 relative, a pair sum over d terms at most
-    d 2^-24 relative), pair sums are added in fp64: 1e-5 relative on each of the three sums covers d = 512 with margin."""
+    """The paper's setting (n = 1000 sounds, d = 512 OpenL3 values) and ragged sizes, both forms of the call.
+    Sorted form (ts_mmd_l1): values on a grid of 2^-32 of the component's largest magnitude, exact integer sums: each of
+    the three sums within 1e-8 relative.  Pairwise form: differences and per-pair sums are fp32 (inputs O(1): each |x - y|
+    carries 2^-24 relative, a pair sum over d terms at most d 2^-24 relative), pair sums are added in fp64: 1e-5
+    relative covers d = 512 with margin."""
     import torch
     rng = np.random.default_rng(n * 1000 + d)
     X = rng.standard_normal((n, d)).astype(np.float32)
     Y = (0.7 * rng.standard_normal((n, d)) + 0.3).astype(np.float32)
-    out = T.ts_mmd_l1(torch.from_numpy(X).cuda(), torch.from_numpy(Y).cuda()).cpu().numpy()
+    if d >= 5:
+        X[:, 1] = 0.0                                                        # a component that is all zeros in one set
+        Y[:, 2] = Y[0, 2]                                                    # a constant component
+        X[:, 3] *= 1e-20                                                     # wildly different scales per component
+        Y[:, 4] *= 1e6                                                       # (on the sorted form's grid: within 2^37 of each other)
+    v, sums = O.mmd_l1(X, Y)
+    Xg, Yg = torch.from_numpy(X).cuda(), torch.from_numpy(Y).cuda()
+    for pairwise, rel in (("sorted", 1e-8), ("pairwise", 1e-5), ("auto", 1e-5)):
+        out = T.ts_mmd_l1(Xg, Yg, form=pairwise).cpu().numpy()
+        for k in range(3):
+            assert out[1 + k] == pytest.approx(sums[k], rel=rel), (pairwise, k)
+        scale = max(sums[0], 1.0) / (n * n)
+        assert abs(out[0] - v) <= 4 * rel * scale, (pairwise, out[0], v)
+        same = T.ts_mmd_l1(Xg, Xg, form=pairwise).cpu().numpy()
+        assert same[0] == 0.0 and same[1] == same[2] == same[3]              # MMD(X, X) = 0 exactly
+        again = T.ts_mmd_l1(Xg, Yg, form=pairwise).cpu().numpy()
+        assert np.array_equal(out, again)                                    # bitwise reproducible
+    # the sorted form does not depend on the order of the rows at all (integer sums); the oracle pins the same invariance
+    perm = rng.permutation(n)
+    a = T.ts_mmd_l1(Xg, Yg, form="sorted").cpu().numpy()
+    b = T.ts_mmd_l1(torch.from_numpy(X[perm]).cuda(), Yg, form="sorted").cpu().numpy()
+    assert np.array_equal(a, b)
+
+
+def test_mmd_l1_large_n_takes_the_pairwise_form(T):
+    """n > 8192 does not fit the sorted form's shared memory: ts_mmd_l1_sorted runs the pairwise kernel (small d keeps the oracle fast)."""
+    import torch
+    rng = np.random.default_rng(9)
+    n, d = 8200, 2
+    X = rng.standard_normal((n, d)).astype(np.float32)
+    Y = (rng.standard_normal((n, d)) + 0.5).astype(np.float32)
+    out = T.ts_mmd_l1(torch.from_numpy(X).cuda(), torch.from_numpy(Y).cuda(), form="sorted").cpu().numpy()
+    ref = T.ts_mmd_l1(torch.from_numpy(X).cuda(), torch.from_numpy(Y).cuda(), form="pairwise").cpu().numpy()
+    assert np.array_equal(out, ref)
     v, sums = O.mmd_l1(X, Y)
     for k in range(3):
         assert out[1 + k] == pytest.approx(sums[k], rel=1e-5)
-    scale = max(sums[0], 1.0) / (n * n)
-    assert abs(out[0] - v) <= 4e-5 * scale, (out[0], v)
-    same = T.ts_mmd_l1(torch.from_numpy(X).cuda(), torch.from_numpy(X).cuda()).cpu().numpy()
-    assert same[0] == 0.0 and same[1] == same[2] == same[3]                  # MMD(X, X) = 0 exactly
-    again = T.ts_mmd_l1(torch.from_numpy(X).cuda(), torch.from_numpy(Y).cuda()).cpu().numpy()
-    assert np.array_equal(out, again)                                        # fixed summation order
 
 
 # ---------------------------------------------------------------------------------- legal end-of-range LFO inputs (H8)
