@@ -188,6 +188,31 @@ int ts_mmd_l1(const float *d_x, const float *d_y, int n, int d, double *d_out);
 int ts_mmd_l1_pairwise(const float *d_x, const float *d_y, int n, int d, double *d_out);
 int ts_mmd_l1_sorted(const float *d_x, const float *d_y, int n, int d, double *d_out);
 
+/* ts_mmd_l1 for callers that cannot allocate device memory at call time.  The three calls above keep their per-CTA
+ * partial sums in a workspace obtained with cudaMalloc (grown on demand, freed by ts_shutdown()).  That does not suit
+ * every host of this library:
+ *   - a process in which another allocator already owns the whole GPU (for example a framework's caching pool that was
+ *     sized to all of HBM), so that a raw cudaMalloc has nothing left to return;
+ *   - a real-time audio or serving loop, where cudaMalloc / cudaFree may synchronise the whole device and take an
+ *     unbounded time in the middle of a deadline;
+ *   - an embedding host (plug-in, sandboxed worker) whose rules forbid allocating after start-up.
+ * ts_mmd_l1_static runs the same kernels as ts_mmd_l1 (the faster form at this n) and returns the same bits, but its
+ * scratch is a fixed array that is part of the library's device image: TS_MMD_STATIC_MAX_PARTIALS doubles = 256 KB,
+ * resident on every GPU that loads libtsynth.so from load to process exit, used or not.  The call itself makes no
+ * cudaMalloc, cudaFree or other allocating call; d_x, d_y and d_out are the caller's, as above.
+ * Limit: max(3 d, 4 (2 T^2 + T)) <= TS_MMD_STATIC_MAX_PARTIALS with T = ceil(n / 64), i.e. n <= 4032 and d <= 10922 (the
+ *   paper's n = 1000, d = 512 needs 2112).  Anything larger: TS_EINVAL with the sizes in ts_last_error(), nothing launched.
+ * First call on a device: it looks up the array's device address (once per device, which must be the current device;
+ *   that is the only set-up).  Make that first call during start-up, before any stream capture begins; later calls only
+ *   launch the two kernels on the ts_set_stream() stream.
+ * Sharing: every call on a device uses the same array and leaves its partial sums there.  Nothing needs clearing between
+ *   calls (each call overwrites every entry it later reads), but two calls that can run on the GPU at the same time --
+ *   different streams, or different host threads -- race on it and give garbage.  Calls issued on one stream are ordered
+ *   and safe.  It does not share anything with ts_mmd_l1's workspace, so those calls may overlap with this one.
+ * Errors: TS_ENULL, TS_EINVAL (n <= 0, d <= 0, n > 65535, beyond the limit), TS_ECUDA. */
+#define TS_MMD_STATIC_MAX_PARTIALS 32768
+int ts_mmd_l1_static(const float *d_x, const float *d_y, int n, int d, double *d_out);
+
 /* Train/test designation of global voice g ("9 * 1024 samples are designated as train, the next 1024
  * samples as test, etc.", i.e. one tenth of the corpus): 1 if (g / 1024) % 10 == 9, else 0.  A position in
  * the corpus, so it is the same for batch size 128 and 1024 (D3).  Host function, no GPU work. */

@@ -32,7 +32,7 @@ EXPORTS = ["ts_sample_params", "ts_render", "ts_render_fmt", "ts_render_host", "
            "ts_corpus_render_fmt", "ts_corpus_render_nebulae", "ts_corpus_open", "ts_corpus_next", "ts_corpus_close", "ts_corpus_is_test", "ts_num_samples",
            "ts_num_ticks", "ts_num_ticks_r", "ts_streaming_lanes", "ts_set_stream", "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes",
            "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_time_kernels", "ts_time_audio_two_streams", "ts_time_fill", "ts_time_alu_bound", "ts_time_pipes", "ts_last_kernel_ms",
-           "ts_last_stats", "ts_render_r", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_mmd_l1_pairwise", "ts_mmd_l1_sorted", "ts_debug_noise_u32", "ts_debug_controls",
+           "ts_last_stats", "ts_render_r", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_mmd_l1_pairwise", "ts_mmd_l1_sorted", "ts_mmd_l1_static", "ts_debug_noise_u32", "ts_debug_controls",
            "ts_debug_phase"]
 TS_F32, TS_F16, TS_BF16 = 0, 1, 2
 
@@ -82,6 +82,7 @@ def lib():
     L.ts_mmd_l1.argtypes = [vp, vp, i32, i32, vp]
     L.ts_mmd_l1_pairwise.argtypes = [vp, vp, i32, i32, vp]
     L.ts_mmd_l1_sorted.argtypes = [vp, vp, i32, i32, vp]
+    L.ts_mmd_l1_static.argtypes = [vp, vp, i32, i32, vp]
     L.ts_corpus_is_test.argtypes = [u64]
     L.ts_num_samples.argtypes = [i32, f64]
     L.ts_num_samples.restype = C.c_int64
@@ -450,6 +451,31 @@ def ts_mmd_l1(x, y, form: str = "auto"):
     _use_current_stream(x.device)
     fn = {"auto": lib().ts_mmd_l1, "pairwise": lib().ts_mmd_l1_pairwise, "sorted": lib().ts_mmd_l1_sorted}[form]
     _check(fn(C.c_void_p(x.data_ptr()), C.c_void_p(y.data_ptr()), int(x.shape[0]), int(x.shape[1]), C.c_void_p(out.data_ptr())))
+    return out
+
+
+MMD_STATIC_MAX_PARTIALS = 32768  # TS_MMD_STATIC_MAX_PARTIALS
+
+
+def ts_mmd_l1_static(x, y, out=None):
+    """ts_mmd_l1 without any device allocation inside the library: for hosts that cannot call cudaMalloc when the call is
+    made (all of the GPU's memory already belongs to another allocator, a real-time loop that cannot afford cudaMalloc's
+    device-wide synchronisation, a host that forbids allocation after start-up).  Same kernels and same bits as
+    ts_mmd_l1(x, y); the scratch is a 256 KB array inside the library's device image, so n <= 4032 and d <= 10922
+    (TsynthError beyond that).  Pass a preallocated CUDA float64 [4] tensor as `out` to keep this wrapper from asking torch
+    for one.  All calls share the scratch: keep them on one stream.  Make the first call (it looks up the array's device
+    address) during start-up."""
+    torch = _torch()
+    if not (x.is_cuda and y.is_cuda and x.dtype == torch.float32 and y.dtype == torch.float32 and x.is_contiguous()
+            and y.is_contiguous() and x.dim() == 2 and tuple(x.shape) == tuple(y.shape)):
+        raise TsynthError("x and y must be contiguous CUDA float32 tensors of the same shape [n, d]")
+    if out is None:
+        out = torch.empty(4, dtype=torch.float64, device=x.device)
+    elif not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 4 and out.device == x.device):
+        raise TsynthError("out must be a contiguous CUDA float64 tensor of 4 elements on the device of x")
+    _use_current_stream(x.device)
+    _check(lib().ts_mmd_l1_static(C.c_void_p(x.data_ptr()), C.c_void_p(y.data_ptr()), int(x.shape[0]), int(x.shape[1]),
+                                  C.c_void_p(out.data_ptr())))
     return out
 
 

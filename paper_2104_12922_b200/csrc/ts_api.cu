@@ -1056,6 +1056,22 @@ int ts_mmd_l1(const float *d_x, const float *d_y, int n, int d, double *d_out) {
 int ts_mmd_l1_pairwise(const float *d_x, const float *d_y, int n, int d, double *d_out) { return mmd_impl(d_x, d_y, n, d, d_out, 1); }
 int ts_mmd_l1_sorted(const float *d_x, const float *d_y, int n, int d, double *d_out) { return mmd_impl(d_x, d_y, n, d, d_out, 2); }
 
+// ts_mmd_l1 for callers that cannot allocate: the scratch is a static device array of ts_mmd.cu (see there and tsynth.h).
+// Touches none of the library's allocated state (S.mmd_ws stays as it is); no cudaMalloc / cudaFree on this path.
+int ts_mmd_l1_static(const float *d_x, const float *d_y, int n, int d, double *d_out) {
+    if (!d_x || !d_y || !d_out) return fail(TS_ENULL, "NULL argument%s");
+    if (n <= 0 || d <= 0 || n > 65535) return fail(TS_EINVAL, "n must be in [1, 65535] and d positive%s");
+    const size_t need = ts_mmd_partial_count(n, d), cap = ts_mmd_static_capacity();
+    if (need > cap) {
+        char detail[160];
+        snprintf(detail, sizeof detail, "n = %d, d = %d needs %zu partial sums, the static scratch holds %zu (n <= 4032 and d <= 10922)",
+                 n, d, need, cap);
+        return fail(TS_EINVAL, "ts_mmd_l1_static: %s; use ts_mmd_l1, which allocates its workspace", detail);
+    }
+    TS_CUDA(ts_launch_mmd_static(d_x, d_y, n, d, d_out, S.lane[0].stream));
+    return TS_OK;
+}
+
 int ts_debug_noise_u32(const uint32_t host_key[2], uint64_t n0, int count, uint32_t *d_out) {
     if (!host_key || !d_out) return fail(TS_ENULL, "NULL argument%s");
     if (count <= 0) return fail(TS_EINVAL, "count must be positive%s");

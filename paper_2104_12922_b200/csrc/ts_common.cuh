@@ -88,6 +88,9 @@ cudaError_t ts_measure_pipes(double host_rates[TS_NPIPES], cudaStream_t st);  //
 // pairwise: 0 = whichever form is faster at this n, 1 = the O(d n^2) tiled form, 2 = the sorted form (n <= 8192, else tiled)
 cudaError_t ts_launch_mmd(const float *d_x, const float *d_y, int n, int d, double *d_partial, double *d_out, int pairwise, cudaStream_t st);
 size_t ts_mmd_partial_count(int n, int d);
+// ts_mmd_l1_static: the faster form with the partial sums in the module's own static device array (no allocation)
+size_t ts_mmd_static_capacity();  // partial sums the array holds (TS_MMD_STATIC_MAX_PARTIALS)
+cudaError_t ts_launch_mmd_static(const float *d_x, const float *d_y, int n, int d, double *d_out, cudaStream_t st);
 // epoch: a value never used before on this `agg` buffer (flags from older launches then read as "not ready")
 // Per-voice setup (S1 optional, S2/S3, derived constants, last audible tick, header).  sample != 0: draw the records
 // first (S1, global voices g0 .. g0 + B - 1 under `seed`) and write them to d_params; else read d_params.

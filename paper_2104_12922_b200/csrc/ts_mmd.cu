@@ -341,3 +341,40 @@ cudaError_t ts_launch_mmd(const float *d_x, const float *d_y, int n, int d, doub
     ts_mmd_final_kernel<<<1, 256, 0, st>>>(d_partial, n, T, d_out);
     return cudaGetLastError();
 }
+
+// ---- ts_mmd_l1_static (tsynth.h): the same two kernels, per-CTA partial sums kept in memory the library image carries --------
+// The partial sums above are the only scratch memory the MMD kernels use.  Some hosts of this library must not (or cannot)
+// ask the CUDA allocator for it at call time: a process whose device memory is entirely owned by another allocator (a
+// framework's caching pool sized to the whole GPU leaves a raw cudaMalloc nothing to hand out), a latency-bound audio or
+// serving loop that cannot take cudaMalloc's implicit device-wide synchronisation, a plug-in running under a host that
+// forbids allocation after start-up.  For them the scratch is this file-scope array: it is part of the loaded module, so
+// every GPU that loads libtsynth.so holds TS_MMD_STATIC_MAX_PARTIALS * 8 bytes (256 KB) of it from module load to exit,
+// whether or not the call is ever made.
+// In HOST code the name `ts_mmd_static_partial` is only a handle for the runtime (a host-side shadow object): its address
+// is not a device address, and a kernel handed `&ts_mmd_static_partial[0]` from host code would fault or write somewhere
+// unrelated.  The device address is looked up once per device with cudaGetSymbolAddress, with that device current.
+static __device__ __align__(256) double ts_mmd_static_partial[TS_MMD_STATIC_MAX_PARTIALS];
+
+constexpr int TS_MMD_MAX_DEVICES = 64;
+static double *ts_mmd_static_ptr[TS_MMD_MAX_DEVICES];  // device address of the array on each device ordinal, NULL = not looked up yet
+
+size_t ts_mmd_static_capacity() { return (size_t)TS_MMD_STATIC_MAX_PARTIALS; }
+
+// The caller has checked ts_mmd_partial_count(n, d) <= ts_mmd_static_capacity().  No cudaMalloc / cudaFree here or below:
+// cudaGetDevice, cudaGetSymbolAddress (first call per device), cudaFuncSetAttribute (first sorted-form launch) and the
+// two kernel launches are all this path calls.  Nothing in the array has to be zero on entry -- the first kernel of a call
+// writes every partial its final kernel reads -- so the previous call's contents are simply overwritten.
+cudaError_t ts_launch_mmd_static(const float *d_x, const float *d_y, int n, int d, double *d_out, cudaStream_t st) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool cached = dev >= 0 && dev < TS_MMD_MAX_DEVICES;
+    double *scratch = cached ? ts_mmd_static_ptr[dev] : nullptr;
+    if (!scratch) {  // set-up: once per device (ordinals past the cache look it up on every call)
+        e = cudaGetSymbolAddress((void **)&scratch, ts_mmd_static_partial);
+        if (e != cudaSuccess) return e;
+        if (!scratch) return cudaErrorInvalidSymbol;
+        if (cached) ts_mmd_static_ptr[dev] = scratch;
+    }
+    return ts_launch_mmd(d_x, d_y, n, d, scratch, d_out, 0, st);
+}
