@@ -300,6 +300,98 @@ def test_d21_lfo_phase_30s_against_exact_rational_sum():
         assert min(d, 1 - d) < 1e-12, (j, d)
 
 
+def test_p6_second_lfo_alone_with_its_own_rate_and_amp_adsrs():
+    """LFO 2 on its own ("two LFOs ... each LFO module includes two dedicated ADSRs"): block h[40..47], amp
+    envelope e = 4 (h[22..26]), rate envelope e = 5 (h[27..31]) per table S2; LFO 1 and its envelopes carry DIFFERENT
+    values, so that reading any of LFO 1's slots instead fails.  Rate ADSR = linear attack over 2 s:
+    f(t) = f0 + dep t / 2  =>  q_j = q0 + sum_{i<j} (f0 + dep i / (2 cr)) / cr (exclusive).  Reverse saw 1 - 2p reads the
+    phase back; mixer source 3 (lfo2) is routed alone into the vco2-pitch row (d = 2)."""
+    h = neutral_h()
+    h[40], h[41], h[42] = 3.0, -4.0, 0.25           # lfo2: frequency, rate-mod depth, initial phase
+    h[43:48] = [0, 0, 0, 0.6, 0]                    # rsaw only
+    h[2 + 5 * 5: 7 + 5 * 5] = [2.0, 0, 1, 0, 1]     # lfo2_rate ADSR (e = 5): A = 2 s, alpha = 1
+    h[2 + 5 * 4: 7 + 5 * 4] = [0.25, 0, 1, 0, 1]    # lfo2_amp  ADSR (e = 4): A = 0.25 s, alpha = 1
+    h[32], h[33], h[34] = 7.0, 9.0, -0.4            # lfo1: everything different
+    h[35:40] = [0, 1, 0, 0, 0]
+    h[2 + 5 * 3: 7 + 5 * 3] = [0.7, 0, 1, 0, 1]     # lfo1_rate ADSR (e = 3)
+    h[2 + 5 * 2: 7 + 5 * 2] = [1.3, 0, 1, 0, 1]     # lfo1_amp  ADSR (e = 2)
+    h[48 + 4 * 2 + 3] = 0.37                        # vco2 pitch row <- lfo2 only
+    N = SR
+    cr = SR / 100
+    E, L, M = O.controls(h, SR, N)
+    j = np.arange(O.num_ticks(N))
+    t = j / cr
+    assert np.allclose(E[5], np.minimum(t / 2.0, 1.0), atol=1e-15)
+    assert np.allclose(E[4], np.minimum(t / 0.25, 1.0), atol=1e-15)
+    q = 0.25 + 3.0 * j / cr - 4.0 * (j * (j - 1) / 2) / (2.0 * cr**2)
+    p = q % 1.0
+    ok = np.minimum(p, 1 - p) > 1e-9                # keep clear of the saw's jump
+    want = np.minimum(t / 0.25, 1.0) * (1 - 2 * p)
+    assert np.allclose(L[1][ok], want[ok], atol=1e-10)
+    assert np.allclose(M[2][ok], want[ok], atol=1e-10)      # one-hot on source 3: the row IS lfo2
+    assert np.all(M[[0, 1, 3, 4]] == 0)
+    assert np.max(np.abs(L[0] - L[1])) > 0.5                # and lfo1 really is something else
+
+
+def test_s7_modmix_every_row_takes_every_source_from_its_own_slot():
+    """w[d][s] = h[48 + 4 d + s] (table S2): a one-hot weight passes source s to row d and to no other row, for all 20
+    (d, s) -- the four sources are made distinct constants / signals first."""
+    base = neutral_h()
+    base[2:7] = [0, 0, 0.25, 0, 1]                  # adsr1 == 0.25
+    base[7:12] = [0, 0, 0.75, 0, 1]                 # adsr2 == 0.75
+    base[32], base[35:40] = 2.0, [0, 0, 1, 0, 0]    # lfo1: 2 Hz saw
+    base[40], base[43:48] = 5.0, [0, 0, 0, 0, 1]    # lfo2: 5 Hz square
+    N = 4000
+    E0, L0, _ = O.controls(base, SR, N)
+    src = [E0[0], E0[1], L0[0], L0[1]]
+    assert np.allclose(src[0], 0.25) and np.allclose(src[1], 0.75) and np.ptp(src[2]) > 0.1 and set(np.unique(src[3])) <= {-1.0, 1.0}
+    for d in range(5):
+        for s_ in range(4):
+            h = base.copy()
+            h[48 + 4 * d + s_] = 0.3
+            E, L, M = O.controls(h, SR, N)
+            assert np.allclose(M[d], src[s_], atol=1e-15), (d, s_)
+            assert np.all(np.delete(M, d, axis=0) == 0), (d, s_)
+    h = base.copy()
+    h[48 + 4 * 4: 48 + 4 * 5] = [1, 0, 0, 3]        # noise-amp row: adsr1 and lfo2, weights 1 : 3
+    E, L, M = O.controls(h, SR, N)
+    assert np.allclose(M[4], (0.25 + 3 * src[3]) / 4, atol=1e-15)
+
+
+def test_s2_default_nebula_value_by_value():
+    """All 78 (lo, hi, curve, symmetric) entries of SURVEY.md 8(c) table S2, typed here from the survey's table (not read
+    from the oracle): time-like parameters c = 0.5, LFO rate c = 0.25, pitch modulation depth c = 0.2 symmetric, tuning
+    and LFO rate-mod depth symmetric, the rest linear."""
+    want = {0: (0, 127, 1, 0), 1: (0.01, 1.0, 0.5, 0)}
+    for e in range(6):
+        b = 2 + 5 * e
+        want[b + 0] = want[b + 1] = want[b + 3] = (0, 2, 0.5, 0)
+        want[b + 2] = (0, 1, 1, 0)
+        want[b + 4] = (0.1, 6, 1, 0)
+    for l in range(2):
+        b = 32 + 8 * l
+        want[b + 0] = (0, 20, 0.25, 0)
+        want[b + 1] = (-10, 10, 0.5, 1)
+        want[b + 2] = (-0.5, 0.5, 1, 0)
+        for i in range(5):
+            want[b + 3 + i] = (0, 1, 1, 0)
+    for i in range(48, 68):
+        want[i] = (0, 1, 1, 0)
+    for v in range(2):
+        b = 68 + 3 * v
+        want[b + 0] = (-24, 24, 1, 1)
+        want[b + 1] = (-96, 96, 0.2, 1)
+        want[b + 2] = (-0.5, 0.5, 1, 0)
+    for i in range(74, 78):
+        want[i] = (0, 1, 1, 0)
+    assert sorted(want) == list(range(78))
+    neb = O.default_nebula()
+    for i in range(78):
+        got = (neb["lo"][i], neb["hi"][i], neb["curve"][i], int(neb["symmetric"][i]))
+        assert got == want[i], (i, got, want[i])
+    assert int(neb["symmetric"].sum()) == 6                                   # 33, 41, 68, 69, 71, 72 and no others
+
+
 def test_s7_modmix_weighted_mean():
     h = neutral_h()
     h[2:7] = [0, 0, 0.25, 0, 1]      # adsr1 == 0.25
