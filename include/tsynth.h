@@ -127,7 +127,10 @@ int ts_corpus_render_nebulae(uint64_t seed, uint64_t first_batch, int n_batches,
  * voice (equal whenever B divides 1024; a batch of 1024-aligned voices never straddles a block).  The call makes the set stream wait
  * for that batch (no host synchronisation) and re-arms the slot handed out by the PREVIOUS call with the batch
  * n_ring - 1 ahead, ordered after everything the caller has queued on the set stream so far: consume a batch on the set
- * stream before asking for the next one.  ts_corpus_close() drains the internal streams. */
+ * stream before asking for the next one.  ts_corpus_close() drains the internal streams.
+ * While an iterator is open the nebula is fixed: ts_set_nebula, ts_corpus_render*, ts_render_r return TS_EINVAL.  If a
+ * batch cannot be issued (TS_ENOMEM, TS_ECUDA), ts_corpus_open / ts_corpus_next drain the internal streams and CLOSE the
+ * iterator before returning that error: there is never a half-open iterator to clean up. */
 typedef struct {
     uint64_t seed;
     int B, sr;
@@ -182,7 +185,12 @@ int ts_render_r(const ts_voice *d_params, int B, int sr, double seconds, int R, 
  *   on a fixed-point grid of 2^-61 of its largest magnitude (an fp32 value is on the grid unless it is 2^37 times smaller
  *   than that maximum) and everything after that is exact integer arithmetic.
  * ts_mmd_l1 runs whichever is faster at this n (the paper's n = 1000, d = 512: sorted, 80 vs 110 us on a B200; n = 4000:
- *   336 vs 1466 us; n = 256: pairwise).  All three are bitwise reproducible and give MMD(X, X) == 0 exactly.
+ *   336 vs 1466 us; n = 256: pairwise).  All three are bitwise reproducible (fixed summation orders).  MMD(X, X) == 0
+ *   EXACTLY is a property of the sorted form (integer sums: the three pair sums of X = Y are the same integer).  The
+ *   pairwise form adds the cross matrix and the two symmetric ones in different orders (all tiles vs doubled upper
+ *   triangle), so its MMD(X, X) is 0 only while the fp64 sums of the fp32 pair sums are still exact (roughly
+ *   24 + log2(n^2) + the dynamic range of the pair sums <= 53 bits); beyond that it is 0 to within fp64 rounding of sums
+ *   of that size.  ts_mmd_l1 runs the pairwise form for n > 8192 and for small n.
  * Errors: TS_ENULL, TS_EINVAL (n <= 0, d <= 0, n > 65535). */
 int ts_mmd_l1(const float *d_x, const float *d_y, int n, int d, double *d_out);
 int ts_mmd_l1_pairwise(const float *d_x, const float *d_y, int n, int d, double *d_out);
@@ -225,7 +233,7 @@ int ts_streaming_lanes(void);                     /* lanes the streaming calls r
 
 int ts_set_stream(void *cuda_stream);              /* cudaStream_t; NULL = legacy default stream   */
 int ts_default_nebula(ts_range host_out78[TS_NPARAM]); /* host copy of the built-in table S2        */
-int ts_set_nebula(const ts_range *host_in78);      /* host table; NULL restores the default.  TS_EINVAL: non-finite entries, curve <= 0, or a negative range for a weight (LFO shapes 35..39, 43..47; modulation mixer 48..67) */
+int ts_set_nebula(const ts_range *host_in78);      /* host table; NULL restores the default.  TS_EINVAL: non-finite entries, curve <= 0, a negative range for a weight (LFO shapes 35..39, 43..47; modulation mixer 48..67), or a corpus iterator is open (its nebula is the one active at ts_corpus_open; close it first) */
 size_t ts_workspace_bytes(int B, int sr, double seconds); /* device bytes ts_render will hold      */
 const char *ts_last_error(void);                   /* host string, owned by the library            */
 int ts_sync(void);                                 /* cudaStreamSynchronize on the set stream; TS_ECUDA if a kernel raised the device error flag */

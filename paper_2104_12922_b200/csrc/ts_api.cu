@@ -428,8 +428,13 @@ int stream_batch(ts_voice *p, sample_spec smp, int B, int sr, double seconds, in
         const uint64_t k = (uint64_t)(n_ring < TS_MAX_RING ? n_ring : TS_MAX_RING);
         if (seq >= k) {
             cudaEvent_t *ev = S.batch_done[(seq - k) % TS_MAX_RING];
+            // lo: the slot's audio; hi: the slot's parameter records, written by the setup kernel of whichever lane the batch
+            // runs on (the old batch's audio finished => its setup kernel, which the audio waited for, finished too)
             for (int x = 0; x < TS_SL; ++x)
-                for (int y = 0; y < TS_SL; ++y) TS_CUDA(cudaStreamWaitEvent(S.lo[x], ev[y], 0));
+                for (int y = 0; y < TS_SL; ++y) {
+                    TS_CUDA(cudaStreamWaitEvent(S.lo[x], ev[y], 0));
+                    TS_CUDA(cudaStreamWaitEvent(S.hi[x], ev[y], 0));
+                }
         }
     }
     const size_t es = fmt_bytes(fmt);
@@ -587,8 +592,10 @@ int ts_corpus_render_fmt(uint64_t seed, uint64_t first_batch, int n_batches, int
     if (rc) return rc;
     rc = fork_streams();
     if (rc) return rc;
-    // Ring hazards: records are written by the setup kernel and read by nothing else on the device; audio slots are
-    // written by the audio kernels, all on `lo` in batch order.  Nothing else to order.
+    // Ring hazards: a slot's records are written by the setup kernel (a `hi` stream) and its audio by the audio kernel (a
+    // `lo` stream) of the lane the batch runs on.  A single-chunk batch in a ring that is a multiple of the lanes always
+    // meets its slot on the same pair of streams (stream order covers it); otherwise stream_batch makes every internal
+    // stream wait for the audio of the batch that used the slot before.
     const size_t es = fmt_bytes(fmt);
     int64_t launches = 0;
     for (int i = 0; i < n_batches && rc == TS_OK; ++i) {
@@ -675,6 +682,16 @@ int ts_corpus_render_nebulae(uint64_t seed, uint64_t first_batch, int n_batches,
     return rc ? rc : rj;
 }
 
+// A batch could not be issued (TS_ENOMEM, TS_ECUDA): the iterator does not stay half open with batches in flight -- the
+// internal streams are drained, the iterator is closed and the first error (code and text) is what the caller sees.
+static int corpus_abort(int rc) {
+    char first[sizeof S.err];
+    memcpy(first, S.err, sizeof first);
+    ts_corpus_close();
+    memcpy(S.err, first, sizeof first);
+    return rc;
+}
+
 int ts_corpus_open(const ts_corpus_cfg *host_cfg, uint64_t first_batch) {
     if (!host_cfg) return fail(TS_ENULL, "host_cfg is NULL%s");
     if (!host_cfg->d_audio_ring || !host_cfg->d_params_ring) return fail(TS_ENULL, "NULL ring%s");
@@ -702,7 +719,7 @@ int ts_corpus_open(const ts_corpus_cfg *host_cfg, uint64_t first_batch) {
     C.open = true;
     for (int i = 0; i < host_cfg->n_ring - 1; ++i) {  // render ahead: every slot but one
         rc = corpus_issue(C.next_render++);
-        if (rc) return rc;
+        if (rc) return corpus_abort(rc);
     }
     return TS_OK;
 }
@@ -720,7 +737,7 @@ int ts_corpus_next(ts_corpus_batch *host_out) {
         TS_CUDA(cudaStreamWaitEvent(S.hi[x], C.consumed, 0));
     }
     const int rc = corpus_issue(C.next_render++);
-    if (rc) return rc;
+    if (rc) return corpus_abort(rc);
     const uint64_t b = C.next_out++;
     const int slot = (int)(b % (uint64_t)C.cfg.n_ring);
     TS_CUDA(cudaStreamWaitEvent(S.lane[0].stream, C.ready[slot], 0));  // the caller's stream waits for this batch
@@ -757,6 +774,10 @@ int ts_default_nebula(ts_range host_out78[TS_NPARAM]) {
 }
 
 int ts_set_nebula(const ts_range *host_in78) {
+    // The iterator's batches are issued without re-uploading the table (corpus_issue -> render_impl on the streaming lanes),
+    // so a change here would split the device table from the host-side extent / silent-tail decisions, and a later
+    // ts_render would upload over a table the iterator's setup kernels are still reading.
+    if (S.corpus.open) return fail(TS_EINVAL, "a corpus iterator is open (its nebula is fixed at ts_corpus_open): close it first%s");
     if (!host_in78) {
         default_nebula(S.nebula);
     } else {

@@ -517,11 +517,42 @@ def test_corpus_iterator_hands_out_audio_params_and_split(T):
         T.ts_corpus_next()                                                   # closed
 
 
+def test_nebula_is_fixed_while_the_iterator_is_open(T):
+    """The iterator issues its batches without re-uploading the nebula, so ts_set_nebula must refuse while it is open (a
+    change would split the device table from the host-side extent / silent-tail decisions: a shorter table would leave
+    ring samples unwritten).  The refused call changes nothing: the batches after it equal plain renders bit for bit."""
+    import torch
+    T.ts_set_nebula(None)
+    B, sr, seconds, first, n_ring = 16, 44100, 0.5, 3, 3
+    N = O.num_samples(sr, seconds)
+    short = T.ts_default_nebula()
+    short["hi"][1] = 0.05                                                    # note duration
+    for e in range(6):
+        short["hi"][2 + 5 * e + 3] = 0.01                                    # every release
+    pr = torch.zeros((n_ring, B, 80), device="cuda")
+    ar = torch.full((n_ring, B, N), 9.0, device="cuda")
+    T.ts_corpus_open(0, first, sr, seconds, T.TS_F32, pr, ar)
+    got = [T.ts_corpus_next()["audio"].clone()]
+    for table in (short, None):
+        with pytest.raises(T.TsynthError, match="iterator is open"):
+            T.ts_set_nebula(table)
+    got += [T.ts_corpus_next()["audio"].clone() for _ in range(4)]
+    T.ts_corpus_close()
+    torch.cuda.synchronize()
+    for k, a in enumerate(got):
+        assert torch.equal(a, T.ts_render(T.ts_sample_params(0, first + k, B), sr, seconds)), k
+    T.ts_set_nebula(short)                                                   # closed: accepted again
+    a = T.ts_render(T.ts_sample_params(0, first, B), sr, seconds)
+    assert not torch.equal(a, got[0])
+    assert not a[:, int(0.07 * sr):].any().item()                            # 0.05 s note + 0.01 s release: silent after that
+    T.ts_set_nebula(None)
+
+
 # ---------------------------------------------------------------------------------- Eq. 2: MMD with the l1 core distance (SURVEY 8(f) item 4)
 @pytest.mark.parametrize("n,d", [(1000, 512), (37, 5), (64, 32), (129, 100), (1, 3), (256, 7), (257, 2), (3000, 16)])
 def test_mmd_l1_against_oracle(T, n, d):
     """The paper's setting (n = 1000 sounds, d = 512 OpenL3 values) and ragged sizes, both forms of the call.
-    Sorted form (ts_mmd_l1): values on a grid of 2^-32 of the component's largest magnitude, exact integer sums: each of
+    Sorted form (ts_mmd_l1_sorted): values on a grid of 2^-61 of the component's largest magnitude, exact integer sums: each of
     the three sums within 1e-8 relative.  Pairwise form: differences and per-pair sums are fp32 (inputs O(1): each |x - y|
     carries 2^-24 relative, a pair sum over d terms at most d 2^-24 relative), pair sums are added in fp64: 1e-5
     relative covers d = 512 with margin."""
