@@ -12,6 +12,7 @@ oracle on the host cores instead.
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import statistics
@@ -36,19 +37,27 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def audio_kernel_source_sha() -> str:
+    """What a stored per-launch counter of the audio kernel is tied to: the kernel's source file."""
+    with open(os.path.join(ROOT, "paper_2104_12922_b200", "csrc", "ts_audio.cu"), "rb") as f:
+        return hashlib.sha256(f.read()).hexdigest()[:16]
+
+
 def ncu_value(name: str, workload: str):
     """A per-launch counter of the audio kernel from the committed summary of the latest `ncu --set full` capture
-    (profiles/<name>.csv: workload,value), if any.  audio_kernel_traffic = dram__bytes_read.sum + dram__bytes_write.sum."""
+    (profiles/<name>.csv: workload,value,sha of csrc/ts_audio.cu at the capture), if any -> (value, stale).  stale: the kernel
+    source has changed since the capture (or the row carries no sha).  audio_kernel_traffic = dram__bytes_read.sum +
+    dram__bytes_write.sum."""
     p = os.path.join(ROOT, "profiles", name + ".csv")
     try:
         with open(p) as f:
             for ln in f:
-                k, _, v = ln.strip().partition(",")
-                if k == workload:
-                    return float(v)
+                cols = ln.strip().split(",")
+                if cols[0] == workload:
+                    return float(cols[1]), not (len(cols) > 2 and cols[2] == audio_kernel_source_sha())
     except Exception:
         pass
-    return None
+    return None, None
 
 
 def cpu_model() -> str:
@@ -170,6 +179,8 @@ def device_records(ts, W, wl, dev):
 
 
 _ALU_PEAK = {}
+MUFU_PER_RUN = 100   # MUFU warp instructions per 20-sample run (profiles/r02_audio_sass_histogram.txt, whole-cycle variant)
+SM_COUNT = 148
 
 
 def alu_peak(ts):
@@ -197,15 +208,32 @@ def kernel_roofline(ts, wl, rec, audio_ring, sm_hz, reps):
     out_bytes = B * N * 4
     achieved = out_bytes / (aud * 1e-3) / 1e9
     peaks = alu_peak(ts)
-    alu_pk = peaks["fastsin"]                                               # the higher of the two: a conservative fraction
-    alu_ach = stats["active_samples"] / (aud * 1e-3)
+    own_pk = peaks["fastsin"]                                               # the higher of the two: a conservative fraction
+    aud_ach = stats["active_samples"] / (aud * 1e-3)                        # audible samples/s of this launch
+    pipes = ts.ts_time_pipes()
+    # The hardware bound of the audible samples: the XU (MUFU) pipe.  A warp renders a 20-sample run of its 32 lanes = 640
+    # samples with MUFU_PER_RUN MUFU warp instructions (SASS histogram, profiles/r02_audio_sass_histogram.txt: SIN for VCO 1,
+    # SIN + COS for the square/saw, EX2 + RCP for the tanh, per sample, in the whole-cycle variant 89 % of the voices take);
+    # ts_time_pipes measures what one MUFU costs a sub-partition (8.0 cycles per warp instruction: 4 lanes per clock).
+    xu_peak = 640.0 / (MUFU_PER_RUN * pipes["MUFU.EX2"]) * 4 * SM_COUNT * sm_hz
+    t_hbm, t_xu = out_bytes / (peak * 1e9), stats["active_samples"] / xu_peak
     return {"audio_kernel_ms": aud, "control_kernel_ms": ctl, "achieved_gbs": achieved, "frac": achieved / peak,
             "peak": peak, "peak_source": peak_src, "active_sample_fraction": active, "chunks": stats["chunks"],
-            "alu_bound": {"bound": "alu", "what": "audible samples/s the SM pipes sustain on the kernel's own sample loop "
-                          "(ts_time_alu_bound, measured in this run: same device function, no memory, no CTA turnover, 8 warps "
-                          "per sub-partition; MUFU.SIN variant; DESIGN.md 5.2)", "achieved": alu_ach, "peak": alu_pk,
-                          "peak_polynomial_sine_variant": peaks["poly"], "unit": "audible samples/s", "frac": alu_ach / alu_pk,
-                          "cycles_per_warp_instruction_per_subpartition": ts.ts_time_pipes()}}
+            "xu_bound": {"bound": "alu", "pipe": "XU (MUFU)", "achieved": aud_ach, "peak": xu_peak, "unit": "audible samples/s",
+                         "frac": aud_ach / xu_peak,
+                         "derivation": f"640 samples per warp-run / ({MUFU_PER_RUN} MUFU per run x {pipes['MUFU.EX2']:.2f} cycles per MUFU warp "
+                                       f"instruction per sub-partition, measured in this run by ts_time_pipes) x 4 sub-partitions x "
+                                       f"{SM_COUNT} SMs x {sm_hz / 1e6:.0f} MHz (SM clock sampled under load)"},
+            "governing_bound": "xu" if t_xu > t_hbm else "hbm",
+            "governing_frac": max(t_hbm, t_xu) / (aud * 1e-3),
+            "governing_frac_note": "max(algorithmic bytes / HBM peak, audible samples / XU bound) / kernel duration: the launch against "
+                                   "whichever hardware bound is the longer for this workload",
+            "own_loop_rate": {"what": "NOT a roofline: audible samples/s of the kernel's own sample loop timed alone (ts_time_alu_bound: "
+                              "same device function, no memory, no CTA turnover, 8 warps per sub-partition; MUFU.SIN variant).  It moves "
+                              "with the code, so `frac` only says how much of the launch is spent outside the loop (headers, table loads, "
+                              "hops, stores, CTA turnover)", "achieved": aud_ach, "rate": own_pk,
+                              "rate_polynomial_sine_variant": peaks["poly"], "unit": "audible samples/s", "frac": aud_ach / own_pk,
+                              "cycles_per_warp_instruction_per_subpartition": pipes}}
 
 
 def measure_config(ts, W, torch, name, dev, sm_hz):
@@ -251,7 +279,8 @@ def measure_config(ts, W, torch, name, dev, sm_hz):
            "ms_per_step": med, "ms_per_step_best": best, "samples_per_s": sps, "x_real_time": sps / sr,
            "audible_samples_per_s": sps * roof["active_sample_fraction"],
            "audio_kernel_ms": roof["audio_kernel_ms"], "control_kernel_ms": roof["control_kernel_ms"], "frac": roof["frac"],
-           "alu_bound_frac": roof["alu_bound"]["frac"], "active_sample_fraction": roof["active_sample_fraction"],
+           "xu_frac": roof["xu_bound"]["frac"], "governing_bound": roof["governing_bound"], "governing_frac": roof["governing_frac"],
+           "own_loop_frac": roof["own_loop_rate"]["frac"], "active_sample_fraction": roof["active_sample_fraction"],
            "step_over_audio_kernel": med / roof["audio_kernel_ms"], "voice_chunks_per_launch": roof["chunks"]}
     del audio_ring
     torch.cuda.empty_cache()
@@ -317,29 +346,37 @@ def run_ours(args, wl):
         two_ms = None
     fill_ms = ts.ts_time_fill(audio_ring, 5)
     fill_gbs = audio_ring.numel() * 4 / (fill_ms * 1e-3) / 1e9
-    traffic = ncu_value("audio_kernel_traffic", wl.name)
+    traffic, traffic_stale = ncu_value("audio_kernel_traffic", wl.name)
     roofline = {"bound": "hbm", "kernel": "ts_audio_kernel<0, TAIL, F32>", "achieved": roof["achieved_gbs"], "peak": roof["peak"],
-                "unit": "GB/s", "frac": roof["frac"], "traffic": traffic,
+                "unit": "GB/s", "frac": roof["frac"],
+                "achieved_is": "ALGORITHMIC bytes per launch (4 B per output sample) / the kernel's launch duration measured in this run; "
+                               "not measured DRAM traffic (that is `traffic`)",
+                "traffic": traffic, "traffic_stale": traffic_stale,
                 "traffic_source": "stored value: dram__bytes_read.sum + dram__bytes_write.sum of one launch in the committed "
-                                  "`ncu --set full` capture (profiles/audio_kernel_traffic.csv), not measured in this run; it is "
+                                  "`ncu --set full` capture (profiles/audio_kernel_traffic.csv, tied to the sha of csrc/ts_audio.cu: "
+                                  "traffic_stale = the kernel source has changed since), not measured in this run; it is "
                                   "below the algorithmic bytes because the 126 MB L2 still holds the end of a single launch's writes",
+                "xu_bound": roof["xu_bound"], "frac_xu": roof["xu_bound"]["frac"],
+                "governing_bound": roof["governing_bound"], "governing_frac": roof["governing_frac"],
+                "governing_frac_note": roof["governing_frac_note"],
                 "peak_source": roof["peak_source"], "algorithmic_bytes_per_launch": out_bytes,
                 "audio_kernel_ms": roof["audio_kernel_ms"], "control_kernel_ms": roof["control_kernel_ms"],
                 "timing": "CUDA events around 50 back-to-back launches of each kernel (ts_time_kernels); control = setup + control",
                 "audio_kernel_ms_two_streams": two_ms,
                 "frac_two_streams": out_bytes / (two_ms * 1e-3) / 1e9 / roof["peak"] if two_ms else None,
-                "alu_frac_two_streams": roof["active_sample_fraction"] * B * N / (two_ms * 1e-3) / roof["alu_bound"]["peak"] if two_ms else None,
+                "own_loop_frac_two_streams": roof["active_sample_fraction"] * B * N / (two_ms * 1e-3) / roof["own_loop_rate"]["rate"] if two_ms else None,
                 "audio_kernel_ms_two_streams_note": "interval / launches with the launches rotating over the audio streams of the streaming lanes, as "
                                                     "the streaming calls issue them: an inverse throughput (the ramp and drain of a launch are "
-                                                    "covered by the other stream), not the launch duration `frac` is computed from; "
-                                                    "frac_two_streams / alu_frac_two_streams are the two bounds on that basis",
+                                                    "covered by the other stream) of AUDIO-ONLY launches with no control kernels competing for the SMs, not the "
+                                                    "launch duration `frac` is computed from and not what the pipeline reaches: that is "
+                                                    "whole_step_frac_of_write_roofline",
                 "store_only_fill_gbs": fill_gbs,
                 "store_only_fill": f"{audio_ring.numel() * 4 >> 20} MiB of 128-bit zero stores, 5 launches (ts_time_fill): what a pure "
                                    "store stream reaches, beside the copy peak above",
-                "active_sample_fraction": roof["active_sample_fraction"], "alu_bound": roof["alu_bound"],
-                "note": "audible samples are bound by the SM pipes (FMA-heavy: Philox IMAD.WIDE + packed fp32; ~46 SASS instructions "
-                        "each), silent tails are pure stores written asynchronously by the audible CTAs; DESIGN.md 5.2 and "
-                        "profiles/r02_audio_bounds.md state the measured ALU bound beside this HBM one",
+                "active_sample_fraction": roof["active_sample_fraction"], "own_loop_rate": roof["own_loop_rate"],
+                "note": "audible samples are bound by the SM pipes (XU: 5 MUFU per sample; FMA-heavy: Philox IMAD.WIDE + packed fp32; ~46 "
+                        "SASS instructions each), silent tails are pure stores written asynchronously by the audible CTAs; the two "
+                        "hardware bounds are `frac` (HBM writes) and `frac_xu` (MUFU pipe), `governing_frac` the launch against the longer",
                 "whole_step_frac_of_write_roofline": (4.0 * value / world / 1e9) / roof["peak"]}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,

@@ -13,6 +13,10 @@
  *     return without synchronising, except ts_render_host(), ts_sync() and ts_shutdown().
  *   - Return value 0 = TS_OK, negative = error; ts_last_error() gives the text.  No exceptions,
  *     no abort(), nothing printed.
+ *   - Hardware behaviour the control stage relies on (reading D28): aligned 16-byte volatile vector accesses
+ *     are single transactions on sm_100 (checked on every read by a doubled epoch field: a torn read is retried, never
+ *     used), and CTAs are dispatched in linear block-index order (not checkable; a violation surfaces as TS_ECUDA
+ *     "look-back timeout" from ts_sync() after a bounded wait, not as wrong audio).
  *   - Not thread-safe: one host thread drives one library instance (one GPU per process).  The library state (nebula,
  *     workspaces, internal streams) is one process-wide singleton: one nebula at a time, one device per process, which
  *     is what one-process-per-GPU launches (torchrun) need.

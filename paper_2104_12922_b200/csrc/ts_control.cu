@@ -178,10 +178,16 @@ constexpr int TS_CTL_IC = TS_CTL_THREADS - 1;  // control intervals per chunk (t
 // A slot is two 16-byte words, each a Q0.64 sum with the launch epoch beside it: one 128-bit store publishes a word,
 // one 128-bit load reads value and flag together (aligned 16-byte accesses are single transactions), so neither side
 // needs a fence -- the same packing CUB's single-word tile descriptors use.
+// What this rests on (reading D28): (i) an aligned 16-byte volatile vector access is ONE memory transaction on
+// sm_100, so value and epoch are never seen half-written -- the PTX memory model itself only promises this per scalar
+// element; (ii) a CTA with a lower linear block index has been dispatched before this one.  (i) is checked, not trusted:
+// the epoch is written into BOTH trailing 32-bit fields of a word (the two ends of the 16 bytes a torn access could
+// split), and a reader takes a word only when both equal the launch epoch -- a torn read spins again instead of being
+// summed.  (ii) cannot be checked from inside; its failure mode is the bounded spin below (TS_ECUDA at the next ts_sync).
 struct __align__(16) ts_agg_word {
     unsigned long long s;
-    unsigned int flag;  // == launch epoch once s is valid
-    unsigned int pad;
+    unsigned int flag;   // == launch epoch once s is valid
+    unsigned int flag2;  // the same epoch again
 };
 struct __align__(16) ts_agg {
     ts_agg_word w[2];
@@ -190,8 +196,8 @@ static_assert(sizeof(ts_agg) == 32, "ts_agg layout");
 
 __device__ __forceinline__ void ts_publish(ts_agg *slot, unsigned long long a, unsigned long long b, unsigned int epoch) {
     uint4 w0, w1;
-    w0.x = (unsigned int)a; w0.y = (unsigned int)(a >> 32); w0.z = epoch; w0.w = 0u;
-    w1.x = (unsigned int)b; w1.y = (unsigned int)(b >> 32); w1.z = epoch; w1.w = 0u;
+    w0.x = (unsigned int)a; w0.y = (unsigned int)(a >> 32); w0.z = epoch; w0.w = epoch;
+    w1.x = (unsigned int)b; w1.y = (unsigned int)(b >> 32); w1.z = epoch; w1.w = epoch;
     asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(&slot->w[0]), "r"(w0.x), "r"(w0.y), "r"(w0.z), "r"(w0.w) : "memory");
     asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(&slot->w[1]), "r"(w1.x), "r"(w1.y), "r"(w1.z), "r"(w1.w) : "memory");
 }
@@ -206,7 +212,7 @@ __device__ __forceinline__ void ts_wait_slot(const ts_agg *p, unsigned int epoch
     for (;;) {  // both words in flight at once: one L2 round trip when the predecessor has already published
         asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v0.x), "=r"(v0.y), "=r"(v0.z), "=r"(v0.w) : "l"(&p->w[0]) : "memory");
         asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v1.x), "=r"(v1.y), "=r"(v1.z), "=r"(v1.w) : "l"(&p->w[1]) : "memory");
-        if (v0.z == epoch && v1.z == epoch) break;
+        if (v0.z == epoch && v0.w == epoch && v1.z == epoch && v1.w == epoch) break;
         __nanosleep(40);
         if (++spins > TS_SPIN_LIMIT) {
             atomicExch(err, 1u);
