@@ -125,6 +125,84 @@ def test_phase_c1(T):
             assert d.max() < 3e-9, (vco, b, d.max())
 
 
+def _fixed_voice(T, h):
+    """Nebula with lo = hi = h[p] (S3 then returns h[p] for any u) on both sides -> (nebula, device records, u, nk) of 2 voices."""
+    neb = np.zeros(O.NPARAM, dtype=O.NEBULA_DTYPE)
+    neb["lo"] = h
+    neb["hi"] = h
+    neb["curve"] = 1.0
+    T.ts_set_nebula(neb)
+    u, nk = O.sample_params(5, 0, 2)
+    return neb, to_dev(u, nk), u, nk
+
+
+def _flat_h(D=100.0):
+    """Everything off / flat (layout S2): all six ADSRs are 1 while t < D, LFOs at 0 Hz, no modulation, no mixer level."""
+    h = np.zeros(O.NPARAM)
+    h[0], h[1] = 69.0, D
+    for e in range(6):
+        h[2 + 5 * e: 7 + 5 * e] = [0.0, 0.0, 1.0, 0.0, 1.0]
+    for l in range(2):
+        h[32 + 8 * l: 40 + 8 * l] = [0.0, 0.0, 0.0, 1.0, 0.0, 0.0, 0.0, 0.0]
+    return h
+
+
+def test_noise_only_voice_pins_reading_d24(T):
+    """S12 defines the noise value as z = (x >> 8) 2^-23 - 1 (exact in fp32); the audio kernel converts the whole word
+    (cvt.rz of x times 2^-31, minus 1: reading D24), which keeps low bits of x that S12 drops (up to 255 x 2^-31 when
+    x < 2^31): |g - a3 z| <= 2^-23 a3 + fp32 rounding, one step of S12's grid.  A voice that is noise alone at a constant gain a3 (noise-amp
+    row <- adsr1 == 1, level l3 = a3 of a level sum of 1, VCO amplitudes 0) isolates it: z is computed here from the oracle's bit-exact
+    Philox words, not from either side's float path."""
+    h = _flat_h()
+    h[48 + 4 * 4 + 0] = 1.0                                                  # noise-amp row <- adsr1 (== 1)
+    a3 = 0.8125                                                              # exact in fp32
+    h[77], h[75] = a3, 1.0 - a3                                              # S13-14 divides by l1 + l2 + l3 (= 1 here); the vco1 amp row is all zero, so l1 adds nothing
+    sr, seconds = 44100, 0.25
+    N = O.num_samples(sr, seconds)
+    try:
+        neb, dev, u, nk = _fixed_voice(T, h)
+        g = T.ts_render(dev, sr, seconds).cpu().numpy().astype(np.float64)
+    finally:
+        T.ts_set_nebula(None)
+    for b in range(2):
+        x = np.array([O.noise_word(nk[b], n) for n in range(N)], dtype=np.uint64)
+        z = (x >> np.uint64(8)).astype(np.float64) * 2.0**-23 - 1.0          # S12, exact
+        err = np.abs(g[b] - a3 * z)
+        assert err.max() <= 2.0**-23 * a3 + 2.0**-24, (b, err.max())         # D24's bound + fp32 rounding of a value <= 1
+        assert err.max() > 0                                                 # and D24 really is a different rounding
+        o = O.render_voice(u[b], nk[b], sr, N, neb)["audio"]
+        assert np.max(np.abs(o - a3 * z)) <= 1e-15                           # the oracle IS S12
+
+
+def test_sine_only_voice_hot_path_recurrence(T):
+    """ts_debug_phase goes through the debug variant of the phase recurrence (P += w; w = fma(w, e1, w)); the hot path uses
+    the pair form (fma(w, c2, P), fma(w, e2, w)).  A unit-gain sine-only voice with a moving pitch (12 semitones of a 3 Hz LFO:
+    every interval has its own geometric increment ratio) reads the hot path's phase back through the sine itself:
+    |dg| = 2 pi |dphi|, so a bound of 1e-6 on the audio -- three orders inside the general 2e-3 -- catches any drift of the
+    pair recurrence above 1.6e-7 cycles.  What lives inside 1e-6: MUFU.SIN (2^-20.5 = 6.8e-7 absolute at worst), the
+    range-reduction multiply (2^-23 relative of <= pi: 3.7e-7 at worst), the gain multiply and the phase grid (2.3e-9 cycles
+    = 1.4e-8); measured worst case on a B200: 4.2e-7."""
+    h = _flat_h()
+    h[32], h[35:40] = 3.0, [1, 0, 0, 0, 0]                                   # lfo1: 3 Hz sine
+    h[48 + 4 * 0 + 2] = 1.0                                                  # vco1 pitch row <- lfo1
+    h[48 + 4 * 1 + 0] = 1.0                                                  # vco1 amp row <- adsr1 (== 1)
+    h[68], h[69], h[70] = 3.5, 12.0, 0.125                                   # tuning, mod depth, initial phase
+    h[75] = 1.0                                                              # level l1
+    sr, seconds = 44100, 2.0
+    N = O.num_samples(sr, seconds)
+    try:
+        neb, dev, u, nk = _fixed_voice(T, h)
+        g = T.ts_render(dev, sr, seconds).cpu().numpy().astype(np.float64)
+    finally:
+        T.ts_set_nebula(None)
+    o = O.render_voice(u[0], nk[0], sr, N, neb, want_phase=True)
+    assert np.max(np.abs(o["audio"] - np.sin(2 * np.pi * o["phase1"]))) <= 1e-12   # the voice is the bare sine of its phase
+    assert np.ptp(np.diff(o["phase1"]) % 1.0) > 1e-3                          # and the increment really moves
+    err = np.abs(g[0] - o["audio"])
+    print("sine-only worst |err|:", err.max(), "at", int(err.argmax()))
+    assert err.max() <= 1e-6, err.max()
+
+
 # ---------------------------------------------------------------------------------- audio parity, all configs
 def test_audio_c1_every_sample(T):
     wl, neb, u, nk, dev = setup_workload(T, "C1")
