@@ -292,6 +292,7 @@ def run_ours(args, wl):
     import paper_2104_12922_b200 as ts
     from paper_2104_12922_b200 import build, shard, workloads as W
     build.build()
+    ts.use_measure_build()   # libtsynth_measure.so: the product's sources + the ts_time_* aids (include/tsynth_measure.h)
     rank, local_rank, world = shard.init("nccl")
     if world != args.gpus:
         raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE is {world}")
@@ -341,7 +342,7 @@ def run_ours(args, wl):
     rec = device_records(ts, W, wl, dev)
     roof = kernel_roofline(ts, wl, rec, audio_ring, sm_hz, 50)
     try:
-        two_ms = min(ts.ts_time_audio_two_streams(rec, sr, seconds, audio_ring, 50) for _ in range(3))
+        two_ms = min(ts.ts_time_audio_lanes(rec, sr, seconds, audio_ring, 50) for _ in range(3))
     except ts.TsynthError:  # the batch needs several voice chunks (C3): the overlapped-launch figure is a one-chunk measurement
         two_ms = None
     fill_ms = ts.ts_time_fill(audio_ring, 5)
@@ -493,33 +494,6 @@ def run_ours(args, wl):
         dist.destroy_process_group()
 
 
-def run_launch_grid(args):
-    """`--launch-grid`: per-launch time of the audio kernel (ts_time_kernels: events around back-to-back launches on one
-    stream) for a series of launch sizes -- 128 voices whose notes outlast the buffer, 0.5 ... 4 s.  Shows that the figure
-    sits on a ~2.05 us grid on this system (profiles/r02_audio_bounds.md section 6).  One JSON line, not a bench value."""
-    import torch
-    import paper_2104_12922_b200 as ts
-    from paper_2104_12922_b200 import build
-    build.build()
-    torch.cuda.set_device(0)
-    dev = torch.device("cuda", 0)
-    neb = ts.ts_default_nebula()
-    neb["lo"][1] = neb["hi"][1] = 4.0          # every voice audible for the whole buffer
-    ts.ts_set_nebula(neb)
-    B, sr, rows = 128, 44100, []
-    rec = ts.ts_sample_params(0, 0, B, device=dev)
-    for k in range(2, 17):
-        seconds = 0.25 * k
-        N = ts.ts_num_samples(sr, seconds)
-        ring = torch.empty((4, B, N), dtype=torch.float32, device=dev)
-        ms = min(ts.ts_time_kernels(rec, sr, seconds, ring, 30)[1] for _ in range(3))
-        rows.append({"seconds": seconds, "tiles": B * (-(-N // 2560)), "audio_kernel_us": round(ms * 1e3, 3)})
-        del ring
-    ts.ts_set_nebula(None)
-    print(json.dumps({"probe": "launch_grid", "what": "audio kernel, us per launch over 30 back-to-back launches on one stream, "
-                      "128 all-audible voices", "series": rows}))
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -530,11 +504,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-configs", action="store_true", help="skip the C1 / C3 / C4 / C5 entries of the line")
-    ap.add_argument("--launch-grid", action="store_true", help="probe: the audio kernel's per-launch time over a series of launch sizes")
     args = ap.parse_args()
-    if args.launch_grid:
-        run_launch_grid(args)
-        return
     args.warmup = max(args.warmup, 3)
     args.repeats = max(args.repeats, 1)
     from paper_2104_12922_b200 import shard, workloads as W

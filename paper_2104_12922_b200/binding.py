@@ -17,7 +17,9 @@ NEBULA_DTYPE = np.dtype([("lo", "<f8"), ("hi", "<f8"), ("curve", "<f8"), ("symme
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libtsynth.so")
+_MEASURE_LIB_PATH = os.path.join(_HERE, "libtsynth_measure.so")
 _lib = None
+_measure = False
 
 
 class TsynthError(RuntimeError):
@@ -31,9 +33,11 @@ class _Out(C.Structure):
 EXPORTS = ["ts_sample_params", "ts_render", "ts_render_fmt", "ts_render_host", "ts_render_host_fmt", "ts_corpus_render",
            "ts_corpus_render_fmt", "ts_corpus_render_nebulae", "ts_corpus_open", "ts_corpus_next", "ts_corpus_close", "ts_corpus_is_test", "ts_num_samples",
            "ts_num_ticks", "ts_num_ticks_r", "ts_streaming_lanes", "ts_set_stream", "ts_default_nebula", "ts_set_nebula", "ts_workspace_bytes",
-           "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_time_kernels", "ts_time_audio_two_streams", "ts_time_fill", "ts_time_alu_bound", "ts_time_pipes", "ts_last_kernel_ms",
+           "ts_last_error", "ts_sync", "ts_shutdown", "ts_set_timing", "ts_last_kernel_ms",
            "ts_last_stats", "ts_render_r", "ts_render_controls", "ts_render_controls_r", "ts_mmd_l1", "ts_mmd_l1_pairwise", "ts_mmd_l1_sorted", "ts_mmd_l1_static", "ts_debug_noise_u32", "ts_debug_controls",
            "ts_debug_phase"]
+# include/tsynth_measure.h: only in libtsynth_measure.so (use_measure_build())
+MEASURE_EXPORTS = ["ts_time_kernels", "ts_time_audio_lanes", "ts_time_fill", "ts_time_alu_bound", "ts_time_pipes"]
 TS_F32, TS_F16, TS_BF16 = 0, 1, 2
 
 
@@ -48,7 +52,17 @@ class _CorpusBatch(C.Structure):
 
 
 def lib_path() -> str:
-    return _LIB_PATH
+    return _MEASURE_LIB_PATH if _measure else _LIB_PATH
+
+
+def use_measure_build() -> None:
+    """Make this process load libtsynth_measure.so INSTEAD of libtsynth.so: the same sources plus the measurement aids of
+    include/tsynth_measure.h (the ts_time_* calls below), so that what bench.py times is the product's own code and the
+    library state (nebula, workspaces, lanes) is one.  Must come before the first library call of the process."""
+    global _measure
+    if _lib is not None and not _measure:
+        raise TsynthError("use_measure_build() must be called before the first library call (libtsynth.so is already loaded)")
+    _measure = True
 
 
 def lib():
@@ -56,10 +70,11 @@ def lib():
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(_LIB_PATH):
-        raise TsynthError(f"{_LIB_PATH} is missing: run `python -m paper_2104_12922_b200.build` "
+    path = lib_path()
+    if not os.path.exists(path):
+        raise TsynthError(f"{path} is missing: run `python -m paper_2104_12922_b200.build` "
                           "(or __graft_entry__.build()); there is no CPU fallback")
-    L = C.CDLL(_LIB_PATH)
+    L = C.CDLL(path)
     vp, u64, i32, f64 = C.c_void_p, C.c_uint64, C.c_int, C.c_double
     L.ts_sample_params.argtypes = [u64, u64, i32, vp]
     L.ts_render.argtypes = [vp, i32, i32, f64, _Out]
@@ -73,10 +88,12 @@ def lib():
     L.ts_corpus_next.argtypes = [C.POINTER(_CorpusBatch)]
     L.ts_num_ticks_r.argtypes = [C.c_int64, i32]
     L.ts_num_ticks_r.restype = C.c_int64
-    L.ts_time_fill.argtypes = [vp, C.c_size_t, i32, vp]
-    L.ts_time_audio_two_streams.argtypes = [vp, i32, i32, f64, vp, i32, i32, vp]
-    L.ts_time_alu_bound.argtypes = [i32, i32, vp]
-    L.ts_time_pipes.argtypes = [vp]
+    if _measure:
+        L.ts_time_fill.argtypes = [vp, C.c_size_t, i32, vp]
+        L.ts_time_audio_lanes.argtypes = [vp, i32, i32, f64, vp, i32, i32, vp]
+        L.ts_time_alu_bound.argtypes = [i32, i32, vp]
+        L.ts_time_pipes.argtypes = [vp]
+        L.ts_time_kernels.argtypes = [vp, i32, i32, f64, vp, i32, i32, vp]
     L.ts_render_controls_r.argtypes = [vp, i32, i32, f64, i32, vp]
     L.ts_render_r.argtypes = [vp, i32, i32, f64, i32, vp]
     L.ts_mmd_l1.argtypes = [vp, vp, i32, i32, vp]
@@ -97,7 +114,6 @@ def lib():
     L.ts_shutdown.restype = None
     L.ts_set_timing.argtypes = [i32]
     L.ts_last_kernel_ms.argtypes = [vp]
-    L.ts_time_kernels.argtypes = [vp, i32, i32, f64, vp, i32, i32, vp]
     L.ts_last_stats.argtypes = [vp]
     L.ts_debug_noise_u32.argtypes = [vp, u64, i32, vp]
     L.ts_debug_controls.argtypes = [vp, i32, i32, f64, vp]
@@ -105,6 +121,14 @@ def lib():
     L.ts_debug_phase.argtypes = [vp, i32, i32, f64, i32, vp]
     _lib = L
     return L
+
+
+def _mlib():
+    """The library, for a ts_time_* call: only the measure build has them."""
+    if not _measure:
+        raise TsynthError("the ts_time_* measurement aids are not in libtsynth.so: call use_measure_build() before the first "
+                          "library call of the process (include/tsynth_measure.h)")
+    return lib()
 
 
 def _check(rc: int):
@@ -191,20 +215,22 @@ def ts_last_kernel_ms():
 
 def ts_time_kernels(params, sr: int, seconds: float, audio_ring, reps: int):
     """-> (control ms, audio ms) per launch, averaged over `reps` back-to-back launches of each kernel."""
+    _mlib()  # refuse before touching CUDA if this process runs the product build
     p = _dev_params(params)
     ms = (C.c_float * 2)()
     _use_current_stream(p.device)
-    _check(lib().ts_time_kernels(C.c_void_p(p.data_ptr()), p.shape[0], sr, float(seconds), C.c_void_p(audio_ring.data_ptr()),
+    _check(_mlib().ts_time_kernels(C.c_void_p(p.data_ptr()), p.shape[0], sr, float(seconds), C.c_void_p(audio_ring.data_ptr()),
                                  int(audio_ring.shape[0]), reps, ms))
     return float(ms[0]), float(ms[1])
 
 
-def ts_time_audio_two_streams(params, sr: int, seconds: float, audio_ring, reps: int) -> float:
+def ts_time_audio_lanes(params, sr: int, seconds: float, audio_ring, reps: int) -> float:
     """-> ms per audio launch when launches rotate over the lanes' audio streams (inverse throughput, not a duration)."""
+    _mlib()  # refuse before touching CUDA if this process runs the product build
     p = _dev_params(params)
     ms = C.c_float()
     _use_current_stream(p.device)
-    _check(lib().ts_time_audio_two_streams(C.c_void_p(p.data_ptr()), p.shape[0], sr, float(seconds), C.c_void_p(audio_ring.data_ptr()),
+    _check(_mlib().ts_time_audio_lanes(C.c_void_p(p.data_ptr()), p.shape[0], sr, float(seconds), C.c_void_p(audio_ring.data_ptr()),
                                            int(audio_ring.shape[0]), reps, C.byref(ms)))
     return float(ms.value)
 
@@ -391,17 +417,19 @@ def ts_corpus_close() -> None:
 
 def ts_time_fill(buf, reps: int) -> float:
     """-> ms per launch of a store-only fill of `buf` (a CUDA tensor)."""
+    _mlib()  # refuse before touching CUDA if this process runs the product build
     ms = C.c_float()
     _use_current_stream(buf.device)
-    _check(lib().ts_time_fill(C.c_void_p(buf.data_ptr()), buf.numel() * buf.element_size(), reps, C.byref(ms)))
+    _check(_mlib().ts_time_fill(C.c_void_p(buf.data_ptr()), buf.numel() * buf.element_size(), reps, C.byref(ms)))
     return float(ms.value)
 
 
 def ts_time_alu_bound(fastsin: bool, reps: int = 64) -> float:
     """-> audible samples/s the SM pipes sustain on the audio kernel's own sample loop (no memory, no CTA turnover)."""
+    _mlib()  # refuse before touching CUDA if this process runs the product build
     v = C.c_double()
     _use_current_stream(_torch().device("cuda", _torch().cuda.current_device()))
-    _check(lib().ts_time_alu_bound(int(fastsin), reps, C.byref(v)))
+    _check(_mlib().ts_time_alu_bound(int(fastsin), reps, C.byref(v)))
     return float(v.value)
 
 
@@ -410,9 +438,10 @@ PIPE_NAMES = ["FFMA", "FFMA2", "IMAD.WIDE.U32", "LOP3", "DFMA", "MUFU.SIN+FMUL",
 
 def ts_time_pipes() -> dict:
     """-> {instruction kind: cycles per warp instruction per SM sub-partition}, each kind issued alone."""
+    _mlib()  # refuse before touching CUDA if this process runs the product build
     r = (C.c_double * 8)()
     _use_current_stream(_torch().device("cuda", _torch().cuda.current_device()))
-    _check(lib().ts_time_pipes(r))
+    _check(_mlib().ts_time_pipes(r))
     return {n: float(r[i]) for i, n in enumerate(PIPE_NAMES)}
 
 

@@ -6,6 +6,9 @@
 #include <string.h>
 
 #include "ts_common.cuh"
+#ifdef TS_MEASURE
+#include "../../include/tsynth_measure.h"
+#endif
 
 namespace {
 
@@ -866,6 +869,7 @@ void ts_shutdown(void) {
     S.math_uploaded = false;
 }
 
+#ifdef TS_MEASURE  // the measurement aids of include/tsynth_measure.h: only in libtsynth_measure.so
 int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, float *d_audio_ring, int n_ring, int reps,
                     float host_ms[2]) {
     if (!d_params || !d_audio_ring || !host_ms) return fail(TS_ENULL, "NULL argument%s");
@@ -923,7 +927,7 @@ int ts_time_kernels(const ts_voice *d_params, int B, int sr, double seconds, flo
     return TS_OK;
 }
 
-int ts_time_audio_two_streams(const ts_voice *d_params, int B, int sr, double seconds, float *d_audio_ring, int n_ring, int reps,
+int ts_time_audio_lanes(const ts_voice *d_params, int B, int sr, double seconds, float *d_audio_ring, int n_ring, int reps,
                               float *host_ms) {
     if (!d_params || !d_audio_ring || !host_ms) return fail(TS_ENULL, "NULL argument%s");
     if (n_ring <= 0 || reps <= 0) return fail(TS_EINVAL, "n_ring and reps must be positive%s");
@@ -1018,6 +1022,7 @@ int ts_time_pipes(double host_rates[8]) {
     TS_CUDA(ts_measure_pipes(host_rates, S.lane[0].stream));
     return TS_OK;
 }
+#endif  // TS_MEASURE
 
 int ts_set_timing(int enable) {
     S.timing = enable != 0;

@@ -393,6 +393,7 @@ ts_audio_r1_kernel(const ts_tick *__restrict__ table, const ts_vhdr *__restrict_
     }
 }
 
+#ifdef TS_MEASURE
 // Measurement aid: the sample loop of the audio kernel (ts_render_run, the same device function) on its own -- no control
 // table, no global stores, no CTA turnover, 8 warps per SM sub-partition -- `reps` runs of 20 samples per thread.  What
 // the SM pipes can do with this instruction mix: the ALU bound of the audible part.
@@ -419,9 +420,11 @@ ts_body_bench_kernel(float *__restrict__ sink, int reps, uint32_t nk0, uint32_t 
     for (int g = 0; g < TS_RUN / 4; ++g) s += my[g].x + my[g].y + my[g].z + my[g].w;
     if (s == 123.456f) sink[threadIdx.x] = s;  // keeps the loop alive; never true in practice
 }
+#endif  // TS_MEASURE
 
 }  // namespace
 
+#ifdef TS_MEASURE
 cudaError_t ts_launch_body_bench(int fastsin, int reps, float *d_sink, cudaStream_t st) {
     static bool attr = false;
     if (!attr) {
@@ -438,6 +441,7 @@ cudaError_t ts_launch_body_bench(int fastsin, int reps, float *d_sink, cudaStrea
         ts_body_bench_kernel<0><<<sms, 1024, 1024 * TS_RUN * 4, st>>>(d_sink, reps, 123u, 456u, 0.4f, 20.f, 0x3f800000u, 1e-3);
     return cudaGetLastError();
 }
+#endif  // TS_MEASURE
 
 cudaError_t ts_launch_audio_r1(const ts_tick *table, const ts_vhdr *hdr, int B, int64_t N, int K, float *audio, cudaStream_t st) {
     const int64_t gx = (N + 511) / 512;

@@ -20,8 +20,8 @@ def L():
     return binding.lib()
 
 
-def declared_symbols():
-    src = open(os.path.join(ROOT, "include", "tsynth.h")).read()
+def declared_symbols(header="tsynth.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(ts_[a-z0-9_]+)\s*\(", src)))
 
@@ -32,6 +32,24 @@ def test_library_exports_every_declared_symbol(L):
     for n in names:
         assert hasattr(L, n), n
     assert sorted(binding.EXPORTS) == names
+
+
+def test_measurement_aids_live_in_their_own_header_and_library(L):
+    """include/tsynth_measure.h <-> libtsynth_measure.so (the same sources + ts_measure.cu with -DTS_MEASURE): that build
+    exports both headers' symbols; the product library exports none of the measurement aids and no bench kernel."""
+    aids = declared_symbols("tsynth_measure.h")
+    assert aids == sorted(binding.MEASURE_EXPORTS) and len(aids) == 5
+    assert not set(aids) & set(declared_symbols())
+    M = ctypes.CDLL(build.LIB_MEASURE)
+    for n in aids + declared_symbols():
+        assert hasattr(M, n), n
+    for n in aids:
+        assert not hasattr(L, n), n
+    blob = open(build.LIB, "rb").read()
+    for needle in (b"ts_time_", b"ts_body_bench_kernel", b"ts_pipe_kernel", b"ts_fill_kernel"):
+        assert needle not in blob, needle
+    with pytest.raises(binding.TsynthError, match="use_measure_build"):
+        binding.ts_time_pipes()                               # this process runs the product build
 
 
 def test_struct_sizes_match_header():

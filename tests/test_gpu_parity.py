@@ -816,27 +816,44 @@ def test_iterator_multi_chunk_batches_odd_ring_fp16(T):
     assert np.all(np.abs(g - o) <= MAX_ABS + 0.5 * ulp16(o, 10))
 
 
+_MEASURE_AIDS_SCRIPT = r"""
+import torch
+import paper_2104_12922_b200 as T
+T.use_measure_build()
+T.ts_set_nebula(None)
+rates = T.ts_time_pipes()
+assert len(rates) == 8 and all(0.9 < v < 20.0 for v in rates.values()), rates
+assert rates["FFMA"] < rates["FFMA2"] < rates["MUFU.EX2"]                # packed fp32x2 is two cycles, MUFU eight
+for fast in (True, False):
+    v = T.ts_time_alu_bound(fast, 16)
+    assert 1e11 < v < 3e12, v                                            # below 148 SMs x 128 lanes x 2 GHz / ~36 instr
+buf = torch.empty(64 << 20, device="cuda", dtype=torch.uint8)
+gbs = buf.numel() / (T.ts_time_fill(buf, 3) * 1e-3) / 1e9
+assert 1000 < gbs < 9000, gbs
+B, sr, seconds = 128, 44100, 4.0
+p = T.ts_sample_params(0, 0, B)
+ring = torch.empty((4, B, T.ts_num_samples(sr, seconds)), device="cuda")
+ctl, aud = T.ts_time_kernels(p, sr, seconds, ring, 10)
+two = T.ts_time_audio_lanes(p, sr, seconds, ring, 10)
+assert 0.005 < two <= aud * 1.05 and 0.005 < ctl < 0.2 and aud < 0.2, (ctl, aud, two)
+assert torch.equal(ring[1], T.ts_render(p, sr, seconds))                 # the timing launches render the real thing
+assert T.lib_path().endswith("libtsynth_measure.so")
+print("MEASURE_AIDS_OK")
+"""
+
+
 def test_measurement_aids_are_sane(T):
-    """ts_time_pipes / ts_time_alu_bound / ts_time_fill / ts_time_audio_two_streams (bench.py's roofline inputs) run and
-    return values in the physically possible range of a B200."""
-    import torch
-    T.ts_set_nebula(None)
-    rates = T.ts_time_pipes()
-    assert len(rates) == 8 and all(0.9 < v < 20.0 for v in rates.values()), rates
-    assert rates["FFMA"] < rates["FFMA2"] < rates["MUFU.EX2"]                # packed fp32x2 is two cycles, MUFU eight
-    for fast in (True, False):
-        v = T.ts_time_alu_bound(fast, 16)
-        assert 1e11 < v < 3e12, v                                            # below 148 SMs x 128 lanes x 2 GHz / ~36 instr
-    buf = torch.empty(64 << 20, device="cuda", dtype=torch.uint8)
-    gbs = buf.numel() / (T.ts_time_fill(buf, 3) * 1e-3) / 1e9
-    assert 1000 < gbs < 9000, gbs
-    B, sr, seconds = 128, 44100, 4.0
-    p = T.ts_sample_params(0, 0, B)
-    ring = torch.empty((4, B, T.ts_num_samples(sr, seconds)), device="cuda")
-    ctl, aud = T.ts_time_kernels(p, sr, seconds, ring, 10)
-    two = T.ts_time_audio_two_streams(p, sr, seconds, ring, 10)
-    assert 0.005 < two <= aud * 1.05 and 0.005 < ctl < 0.2 and aud < 0.2, (ctl, aud, two)
-    assert torch.equal(ring[1], T.ts_render(p, sr, seconds))                 # the timing launches render the real thing
+    """ts_time_pipes / ts_time_alu_bound / ts_time_fill / ts_time_kernels / ts_time_audio_lanes (bench.py's roofline inputs,
+    include/tsynth_measure.h) run and return values in the physically possible range of a B200.  They live in
+    libtsynth_measure.so only, which a process loads INSTEAD of the product library: a process of its own, as bench.py is."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", _MEASURE_AIDS_SCRIPT], cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "MEASURE_AIDS_OK" in r.stdout, r.stdout[-2000:] + r.stderr[-4000:]
+    with pytest.raises(T.TsynthError, match="use_measure_build"):
+        T.ts_time_pipes()                                                    # not in the product library this process runs
 
 
 # ---------------------------------------------------------------------------------- a randomised sweep at the bench's own shape
