@@ -448,12 +448,28 @@ def run_ours(args, wl):
         T = -(-n // 64)
         pair_comps = (T * T + T * (T + 1)) * 64 * 64 * d                 # (pair, component) items computed, padded tiles included
         alu_s = 2.0 * pair_comps / (148 * 128 * sm_hz)                    # 2 FADD-class thread instructions per item
+        # the sorted form (the one ts_mmd_l1 runs at this n): a bitonic network of M = 2^L keys per component has (M / 2) L (L + 1) / 2
+        # compare-exchanges; one 64-bit compare-exchange is ~11 integer instructions (profiles/r02_final.md) on the half-rate
+        # integer pipe, whose cost per warp instruction per sub-partition is measured in this run (ts_time_pipes: LOP3)
+        M = 512
+        while M < 2 * n:
+            M *= 2
+        Lg = M.bit_length() - 1
+        cmpx = d * (M // 2) * Lg * (Lg + 1) // 2
+        int_cycles = roof["own_loop_rate"]["cycles_per_warp_instruction_per_subpartition"]["LOP3"]
+        sort_s = (cmpx / 32.0) * 11.0 * int_cycles / (4 * SM_COUNT) / sm_hz
         line["mmd_l1"] = {"ms_per_call": mmd["auto"], "ms_pairwise_form": mmd["pairwise"], "ms_sorted_form": mmd["sorted"],
                           "n": n, "d": d, "bound": "alu", "unit": "s", "peak_s": alu_s, "frac": alu_s / (mmd["pairwise"] * 1e-3),
+                          "sorted_form": {"bound": "alu", "pipe": "integer (half rate)", "peak_s": sort_s, "frac": sort_s / (mmd["sorted"] * 1e-3),
+                                          "derivation": f"{cmpx} compare-exchanges of 64-bit keys ({d} components x {M // 2} x {Lg * (Lg + 1) // 2} "
+                                                        f"network levels) / 32 lanes x ~11 integer instructions x {int_cycles:.2f} cycles per warp "
+                                                        f"instruction per sub-partition (measured) / {4 * SM_COUNT} sub-partitions / SM clock; the "
+                                                        "strided loads, the 128-bit scan and the reductions (a quarter of the kernel's instructions) "
+                                                        "are not in the bound"},
                           "what": "Eq. 2 with the l1 core distance (P:L230).  ts_mmd_l1 runs the faster of two forms: pairwise "
-                                  "(O(d n^2); `bound` / `frac` are this form's: 2 FADD-class instructions per (pair, component) at 148 SMs "
-                                  "x 128 fp32 lanes per clock) and sorted (O(d n log^2 n): one bitonic sort of the 2n values of every "
-                                  "component in shared memory, exact integer sums); embeddings (4 MB) are L2-resident"}
+                                  "(O(d n^2); the top-level `bound` / `frac` are this form's: 2 FADD-class instructions per (pair, component) at 148 SMs "
+                                  "x 128 fp32 lanes per clock) and sorted (`sorted_form` carries its own bound: (O(d n log^2 n): one bitonic sort of the 2n values of every "
+                                  "component in shared memory, exact integer sums)); embeddings (4 MB) are L2-resident"}
         # ---- a nebula sweep in the shape of the paper's tuning runs (256 sounds per candidate table)
         import numpy as np
         nt, Bn = 24, 256

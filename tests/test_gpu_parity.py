@@ -757,6 +757,39 @@ def test_lookback_stress_bitwise_repeatable(T):
     T.ts_set_nebula(None)
 
 
+def test_lookback_deep_chain_under_saturating_audio_of_other_lanes(T):
+    """The tightest residency the streaming path can produce for the look-back (reading D28): 30 s batches at 48 kHz whose
+    notes are held to the end (duration lo = hi = 30 s: every one of the 114 chunks per voice is audible, none is skipped),
+    streamed over the three lanes, so that the 114-chunk chain of batch i + 1 is dispatched under the saturating audio
+    launches of batches i and i - 1.  Integer carries: a missed, stale or torn aggregate changes bits.  40 repeats must
+    reproduce the first result bit for bit, equal the single-call render, and raise no look-back timeout."""
+    import torch
+    neb = T.ts_default_nebula()
+    neb["lo"][1] = neb["hi"][1] = 30.0
+    T.ts_set_nebula(neb)
+    try:
+        B, sr, sec, nb = 8, 48000, 30.0, 6
+        N = T.ts_num_samples(sr, sec)
+        pr = torch.empty((3, B, 80), device="cuda")
+        ar = torch.empty((3, B, N), device="cuda")
+        T.ts_corpus_render(4, 10, nb, sr, sec, pr, ar)
+        torch.cuda.synchronize()
+        ref = ar.clone()
+        assert ref[:, :, -480:].abs().max().item() > 0                       # held to the end: the last chunk is audible
+        for slot in range(3):
+            i = slot + 3                                                     # batches 3, 4, 5 are what the ring holds
+            assert torch.equal(ref[slot], T.ts_render(T.ts_sample_params(4, 10 + i, B), sr, sec)), slot
+        for it in range(40):
+            if it % 10 == 0:
+                ar.fill_(7.0)
+            T.ts_corpus_render(4, 10, nb, sr, sec, pr, ar)
+            torch.cuda.synchronize()
+            assert torch.equal(ar, ref), it
+        T.ts_sync()                                                          # raises if a look-back wait gave up
+    finally:
+        T.ts_set_nebula(None)
+
+
 def test_audio_rate_control_mode_r1(T):
     """SURVEY 8(f) item 3, the R = 1 mode of the AUDIO path (reading D27): every sample is a control tick.  Against the
     oracle's render_voice_r(R = 1) on C2's first voices at C2's length (176 401 ticks per voice), plus a ragged case; and
